@@ -1,0 +1,273 @@
+"""Pins of the whole spatial operator of the oracle (P5 exact solutions, P7, P8, P9, P14): the residual must
+converge spectrally to the analytic time derivative of exact (nonlinear) solutions of Eq. 1-10, the BR1 gradient
+must be exact for polynomials, the polytrope must be in hydrostatic balance, and a brute-force evaluation of
+Eq. 21-24 on one element must reproduce the 1-D-operator path."""
+import numpy as np
+import pytest
+
+from oracle import binding as ob
+from paper_2502_17805_b200 import inputs as I
+
+GAM = 5.0 / 3.0
+
+
+def box_oracle(n, shape, phys, lengths=(1.0, 1.0, 1.0), distort=0.0, walls_z=False):
+    m = I.periodic_box(*shape, lengths, I.lobatto_abscissae(n + 1), distort=distort, walls_z=walls_z)
+    o = ob.Oracle(m, n, phys)
+    return o, o.geometry()["xsol"], m
+
+
+def rel_err(r, ref):
+    return np.abs(r - ref).reshape(9, -1).max(1) / max(np.abs(ref).max(), 1e-300)
+
+
+# ------------------------------------------------------------------------------- exact ideal solutions
+def density_advection(x):
+    U = np.array([0.4, -0.3, 0.2]); B = np.array([0.3, 0.5, -0.2]); k = 2 * np.pi * np.array([1.0, 1.0, 1.0])
+    ph = k[0] * x[0] + k[1] * x[1] + k[2] * x[2]
+    rho = 1.0 + 0.2 * np.sin(ph)
+    one = np.ones_like(rho)
+    Q = I.conserved(rho, U[:, None, None] * one, one, B[:, None, None] * one, 0 * one, GAM)
+    drho_dt = -(U @ k) * 0.2 * np.cos(ph)
+    dQ = np.zeros_like(Q)
+    dQ[0] = drho_dt
+    for i in range(3):
+        dQ[1 + i] = U[i] * drho_dt
+    dQ[4] = 0.5 * (U @ U) * drho_dt
+    return Q, dQ
+
+
+def alfven_wave(x, t=0.0, A=0.1, B0=1.0, rho0=1.0, p0=1.0):
+    """Circularly polarised Alfven wave (exact nonlinear solution of ideal MHD) travelling along (1,1,0)/sqrt2,
+    oblique to the box axes.  Returns Q and dQ/dt."""
+    s2 = np.sqrt(2.0)
+    e0 = np.array([1, 1, 0]) / s2; e1 = np.array([-1, 1, 0]) / s2; e2 = np.array([0, 0, 1.0])
+    k = 2 * np.pi * s2
+    vA = B0 / np.sqrt(rho0)
+    ph = k * ((x[0] + x[1]) / s2 - vA * t)
+    c, s = np.cos(ph), np.sin(ph)
+    one = np.ones_like(c)
+    Bp = A * (c[None] * e1[:, None, None] + s[None] * e2[:, None, None])
+    dBp = -vA * k * A * (-s[None] * e1[:, None, None] + c[None] * e2[:, None, None])
+    B = B0 * e0[:, None, None] * one + Bp
+    U = -Bp / np.sqrt(rho0)
+    Q = I.conserved(rho0 * one, U, p0 * one, B, 0 * one, GAM)
+    dQ = np.zeros_like(Q)
+    dQ[1:4] = -np.sqrt(rho0) * dBp
+    dQ[5:8] = dBp
+    return Q, dQ
+
+
+def glm_wave(x, c_h, a=0.05, B0=0.4):
+    """Right-going GLM wave B_x = B0 + f(x - c_h t), psi = f: exact for U = 0 with the Powell sources of Eq. 5."""
+    f = a * np.sin(2 * np.pi * x[0]); df = a * 2 * np.pi * np.cos(2 * np.pi * x[0])
+    one = np.ones_like(f)
+    B = np.stack([B0 + f, 0.3 * one, -0.2 * one])
+    Q = I.conserved(one, np.zeros((3,) + f.shape), one, B, f, GAM)
+    dQ = np.zeros_like(Q)
+    dQ[5] = -c_h * df
+    dQ[8] = -c_h * df
+    dQ[4] = (B[0] + f) * (-c_h * df)
+    return Q, dQ
+
+
+@pytest.mark.parametrize("case", ["advection", "alfven", "glm"])
+def test_p5_residual_converges_to_exact_time_derivative(case):
+    c_h = 1.3
+    phys = I.Physics(c_h=c_h, flags=I.FLAG_POWELL)
+    errs = []
+    for n in (4, 6, 8):
+        o, x, _ = box_oracle(n, (3, 3, 3), phys, distort=0.05)
+        Q, dQ = {"advection": density_advection, "alfven": alfven_wave, "glm": lambda xx: glm_wave(xx, c_h)}[case](x)
+        o.set_state(Q)
+        errs.append(rel_err(o.residual(), dQ).max())
+    assert errs[1] < 0.1 * errs[0] and errs[2] < 0.1 * errs[1], errs       # spectral convergence in n
+    assert errs[2] < 2e-3, errs
+
+
+def test_p5_energy_row_needs_the_glm_term():
+    """Reading G6: without C_h psi B in the energy flux the GLM wave's energy equation would be off by O(1)."""
+    c_h = 1.3
+    o, x, _ = box_oracle(8, (4, 1, 1), I.Physics(c_h=c_h, flags=I.FLAG_POWELL))
+    Q, dQ = glm_wave(x, c_h)
+    o.set_state(Q)
+    r = o.residual()
+    assert np.abs(dQ[4]).max() > 0.05                         # the term is not small ...
+    assert np.abs(r[4] - dQ[4]).max() < 1e-4 * np.abs(dQ[4]).max()      # ... and is reproduced
+
+
+# ------------------------------------------------------------------------------- diffusion operators
+def test_p7_shear_resistive_and_thermal_decay_rates():
+    """Residual of single Fourier modes equals -(diffusivity) k^2 * mode (exact for these uniform-density fields):
+    shear wave (Eq. 8), resistive decay (Eq. 7 induction row, sign of G10), heat conduction with kappa and kappa_r (Eq. 9)."""
+    n = 8
+    nu, kap, eta, kr = 0.013, 0.021, 0.017, 0.009
+    phys = I.Physics(R_gas=1.3, Cp=GAM * 1.3 / (GAM - 1), nu=nu, kappa=kap, eta=eta, kr_scale=kr, kr_c=(1.0, 0.0, 0.0),
+                     c_h=1.0, flags=I.FLAG_DIFFUSION)
+    o, x, _ = box_oracle(n, (6, 1, 1), phys)
+    k = 2 * np.pi
+    sx, one = np.sin(k * x[0]), np.ones_like(x[0])
+    zero3 = np.zeros((3,) + one.shape)
+    eps = 1e-5
+    # (a) shear wave u_y = eps sin(kx): d/dt(rho u_y) = -nu k^2 rho u_y
+    U = zero3.copy(); U[1] = eps * sx
+    o.set_state(I.conserved(1.5 * one, U, one, zero3, 0 * one, GAM))
+    r = o.residual()
+    np.testing.assert_allclose(r[2], -nu * k * k * 1.5 * eps * sx, rtol=0, atol=1e-5 * nu * k * k * 1.5 * eps)
+    # (b) B_y = eps sin(kx): dB_y/dt = -eta k^2 B_y
+    B = zero3.copy(); B[1] = eps * sx
+    o.set_state(I.conserved(1.5 * one, zero3, one, B, 0 * one, GAM))
+    r = o.residual()
+    np.testing.assert_allclose(r[6], -eta * k * k * eps * sx, rtol=0, atol=1e-5 * eta * k * k * eps)
+    # (c) p = 1 + eps sin(kx), rho uniform, U = 0: dE/dt = -(kappa Cp/(gamma R) + kappa_r Cp/R) k^2 eps sin(kx)
+    o.set_state(I.conserved(1.5 * one, zero3, 1 + eps * sx, zero3, 0 * one, GAM))
+    r = o.residual()
+    rate = (kap * phys.Cp / (GAM * phys.R_gas) + kr * phys.Cp / phys.R_gas) * k * k
+    np.testing.assert_allclose(r[4], -rate * eps * sx, rtol=0, atol=1e-5 * eps * rate)
+
+
+# ------------------------------------------------------------------------------- BR1 gradient
+def test_p8_gradient_exact_for_polynomials_and_spectral_on_shell():
+    n = 5
+    o, x, m = box_oracle(n, (3, 3, 3), I.Physics())
+    c = 13                                                     # central element: all neighbours see the same polynomial
+    rng = np.random.default_rng(3)
+    Q = np.zeros(o.shape)
+    coef = rng.normal(size=(9, n, n, n))
+    dref = np.zeros((9, 3) + x.shape[1:])
+    for v in range(9):
+        for a in range(n):
+            for b in range(n):
+                for cc in range(n):
+                    if a + b + cc > n - 1:
+                        continue
+                    w = coef[v, a, b, cc]
+                    Q[v] += w * x[0] ** a * x[1] ** b * x[2] ** cc
+                    if a: dref[v, 0] += w * a * x[0] ** (a - 1) * x[1] ** b * x[2] ** cc
+                    if b: dref[v, 1] += w * b * x[0] ** a * x[1] ** (b - 1) * x[2] ** cc
+                    if cc: dref[v, 2] += w * cc * x[0] ** a * x[1] ** b * x[2] ** (cc - 1)
+    o.set_state(Q)
+    G = o.gradient().reshape(9, 3, *x.shape[1:])
+    np.testing.assert_allclose(G[:, :, c], dref[:, :, c], atol=1e-11 * np.abs(dref).max())
+    # smooth field on the curved shell: spectral convergence
+    errs = []
+    for nn in (4, 6):
+        ms = I.cubed_sphere_shell(3, 3, 0.7, 0.95, I.lobatto_abscissae(nn + 1))
+        os_ = ob.Oracle(ms, nn, I.Physics())
+        xs_ = os_.geometry()["xsol"]
+        Q = np.zeros(os_.shape)
+        Q[0] = np.sin(2 * xs_[0]) * np.cos(xs_[1]) + xs_[2] ** 2
+        Q[1:] = 1.0
+        os_.set_state(Q)
+        G = os_.gradient()
+        mid = (np.arange(ms["n_elem"]) // 9) % 3 == 1          # away from the walls (Q_b is not the field there)
+        ex = [2 * np.cos(2 * xs_[0]) * np.cos(xs_[1]), -np.sin(2 * xs_[0]) * np.sin(xs_[1]), 2 * xs_[2]]
+        errs.append(max(np.abs(G[p][mid] - ex[p][mid]).max() for p in range(3)))
+    assert errs[1] < 0.05 * errs[0] and errs[1] < 1e-3, errs
+
+
+# ------------------------------------------------------------------------------- sources
+def test_p9_polytrope_is_in_hydrostatic_balance():
+    """Eq. 25-27: the momentum residual of the polytrope vanishes spectrally (relative to rho*g)."""
+    errs = []
+    for n in (4, 6):
+        sh = I.Shell(N_rho=3.0)
+        m = I.cubed_sphere_shell(3, 3, sh.r_b, sh.r_t, I.lobatto_abscissae(n + 1))
+        o = ob.Oracle(m, n, I.Physics(GM=1.0, c_h=1.0, flags=I.FLAG_GRAVITY))
+        x = o.geometry()["xsol"]
+        r = np.sqrt((x ** 2).sum(0))
+        rho, p, T = sh.profile(r)
+        zero3 = np.zeros((3,) + r.shape)
+        o.set_state(I.conserved(rho, zero3, p, zero3, 0 * r, sh.gamma))
+        R = o.residual()
+        errs.append((np.abs(R[1:4]).max(0) / (rho / r ** 2)).max())
+        # U = 0: mass / energy residuals are only the Rusanov dissipation on the (spectrally small) interface jumps
+        assert np.abs(R[0]).max() < 3 * errs[-1] and np.abs(R[4]).max() < 3 * errs[-1]
+    assert errs[1] < 0.02 * errs[0] and errs[1] < 1e-4, errs
+    # the stratification has the requested number of density scale heights
+    rb, _, _ = sh.profile(sh.r_b); rt, _, _ = sh.profile(sh.r_t)
+    assert abs(np.log(rb / rt) - 3.0) < 1e-12
+
+
+def test_p9_coriolis_and_glm_damping_act_pointwise():
+    n = 4
+    phys = I.Physics(Omega=0.7, a_psi=3.0, c_h=0.0, flags=I.FLAG_CORIOLIS | I.FLAG_GLM_DAMP)
+    o, x, _ = box_oracle(n, (2, 2, 2), phys)
+    one = np.ones_like(x[0])
+    U = np.stack([0.3 * one, -0.2 * one, 0.1 * one])
+    Q = I.conserved(1.4 * one, U, one, np.zeros_like(U), 0.25 * one, GAM)
+    o.set_state(Q)
+    R = o.residual()
+    np.testing.assert_allclose(R[1], 2 * 1.4 * 0.7 * (-0.2), atol=1e-12)       # -2 rho Omega x U
+    np.testing.assert_allclose(R[2], -2 * 1.4 * 0.7 * 0.3, atol=1e-12)
+    np.testing.assert_allclose(R[8], -3.0 * 0.25, atol=1e-12)                    # psi' = -a psi
+    np.testing.assert_allclose(R[[0, 3, 4, 5, 6, 7]], 0.0, atol=1e-12)
+
+
+# ------------------------------------------------------------------------------- brute force (P14)
+def test_p14_bruteforce_single_element_divergence():
+    """Evaluate Eq. 22-24 as literal triple sums with analytically differentiated basis polynomials
+    (numpy.polynomial) on one curved periodic element and compare with the oracle's residual."""
+    n = 4
+    c_h = 0.9
+    phys = I.Physics(c_h=c_h, flags=0)
+    o, x, m = box_oracle(n, (1, 1, 1), phys, distort=0.1)
+    geo = o.geometry()
+    rng = np.random.default_rng(5)
+    sh = x.shape[1:]
+    Q = I.conserved(1 + 0.1 * rng.uniform(-1, 1, sh), 0.2 * rng.uniform(-1, 1, (3,) + sh), 1 + 0.1 * rng.uniform(-1, 1, sh),
+                    0.3 * rng.uniform(-1, 1, (3,) + sh), 0.1 * rng.uniform(-1, 1, sh), GAM)
+    o.set_state(Q)
+    R = o.residual()
+    xs, xf = ob.nodes(n)
+    P = np.polynomial.Polynomial
+
+    def basis(nodes, i):
+        others = np.delete(nodes, i)
+        return P.fromroots(others) / np.prod(nodes[i] - others)
+    h = [basis(xs, i) for i in range(n)]
+    l = [basis(xf, i) for i in range(n + 1)]
+    Qe = Q[:, 0].reshape(9, n, n, n)                              # [v,k,j,i]
+    S = geo["S"][0]                                               # [fam,comp,nf]
+    N1 = n + 1
+    # Q at the flux points by Eq. 21 (literal sums), fluxes by the pinned pointwise functions
+    Ft = [np.zeros((9, n, n, N1)), np.zeros((9, n, N1, n)), np.zeros((9, N1, n, n))]
+    Qh = [np.einsum("vkji,mi->vkjm", Qe, np.array([[h[i](xf[mm]) for i in range(n)] for mm in range(N1)])),
+          np.einsum("vkji,mj->vkmi", Qe, np.array([[h[i](xf[mm]) for i in range(n)] for mm in range(N1)])),
+          np.einsum("vkji,mk->vmji", Qe, np.array([[h[i](xf[mm]) for i in range(n)] for mm in range(N1)]))]
+    for d in range(3):
+        Sd = S[d].reshape((3,) + Ft[d].shape[1:])
+        it = np.ndindex(*Ft[d].shape[1:])
+        for idx in it:
+            mm = idx[2 - d]
+            q = Qh[d][(slice(None),) + idx]
+            s = Sd[(slice(None),) + idx]
+            if 0 < mm < n:
+                Ft[d][(slice(None),) + idx] = ob.flux_inviscid(phys, q, s)
+            else:
+                jdx = list(idx); jdx[2 - d] = n - mm               # periodic single element: neighbour = opposite face
+                qo = Qh[d][(slice(None),) + tuple(jdx)]
+                sg = 1.0 if mm == n else -1.0
+                area = np.linalg.norm(s)
+                Ft[d][(slice(None),) + idx] = sg * area * ob.flux_rusanov(phys, q, qo, sg * s / area)
+    detJ = geo["detJ"][0].reshape(n, n, n)
+    Rb = np.zeros((9, n, n, n))
+    for kk in range(n):
+        for jj in range(n):
+            for ii in range(n):
+                X, Y, Z = xs[ii], xs[jj], xs[kk]
+                div = np.zeros(9)
+                for k2 in range(n):            # Eq. 22: dF~/dxi = sum F_ijk l_i'(xi) h_j(eta) h_k(zeta)
+                    for j2 in range(n):
+                        for i2 in range(N1):
+                            div += Ft[0][:, k2, j2, i2] * l[i2].deriv()(X) * h[j2](Y) * h[k2](Z)
+                for k2 in range(n):            # Eq. 23
+                    for j2 in range(N1):
+                        for i2 in range(n):
+                            div += Ft[1][:, k2, j2, i2] * h[i2](X) * l[j2].deriv()(Y) * h[k2](Z)
+                for k2 in range(N1):           # Eq. 24
+                    for j2 in range(n):
+                        for i2 in range(n):
+                            div += Ft[2][:, k2, j2, i2] * h[i2](X) * h[j2](Y) * l[k2].deriv()(Z)
+                Rb[:, kk, jj, ii] = -div / detJ[kk, jj, ii]        # Eq. 16 divided by |J|
+    np.testing.assert_allclose(R[:, 0], Rb.reshape(9, -1), atol=1e-11 * np.abs(Rb).max())

@@ -1,0 +1,119 @@
+/* chorus.h -- C ABI of the B200-native CHORUS-MHD hot path (libchorus_b200.so).
+ *
+ * The hot path is the per-stage spectral-difference (SD) residual of the compressible MHD equations with
+ * GLM divergence cleaning on curved hexahedra, plus the explicit SSPRK(5,3) update, as defined in
+ * arxiv 2502.17805 (citations: PAPER.md:<line>, section / equation).  Every step runs in hand-written CUDA
+ * kernels for sm_100a; there is no CPU fallback: every entry point fails with CHORUS_ECUDA when no device
+ * is usable.  No torch types cross this boundary: plain pointers (HOST or DEVICE as stated) and sizes.
+ *
+ * Conventions
+ *   n = order = solution points per direction; n^3 solution points (Chebyshev-Gauss, Eq. 18),
+ *   n+1 flux points per direction (Legendre roots of P_{n-1} plus 0 and 1), three staggered
+ *   flux families of n^2 (n+1) points.
+ *   Variables (Eq. 2): rho, rho*u, rho*v, rho*w, E, Bx, By, Bz, psi -- 9 fp64 per point.
+ *   state / residual layout  [9][n_elem][n^3]            i (xi) fastest, then j (eta), then k (zeta)
+ *   gradient layout          [27][n_elem][n^3]           row 3*v+p = d Q_v / d x_p
+ *   family-d layout          n^2 (n+1) per element: natural (k,j,i) order with axis d extended to n+1
+ *   Faces 0..5 = xi0, xi1, eta0, eta1, zeta0, zeta1; a face point is (a,b) = the two remaining axes in
+ *   increasing order.  Orientation code (bit0 swap a<->b, bit1 reverse a, bit2 reverse b, applied in that
+ *   order) maps an own face point (a,b) to the coinciding neighbour face point (a',b').
+ *
+ * Ownership: the caller owns every buffer it passes.  chorus_init copies the mesh; the library owns all
+ * device arrays until chorus_free.  One opaque context per mesh; no global state; contexts are not
+ * thread-safe.  All work is enqueued on the cudaStream_t given to chorus_init; calls that take or return
+ * HOST data synchronise that stream, calls with on_device = 1 are asynchronous on it.
+ *
+ * Errors: every function returns 0 (CHORUS_OK) or a negative code; chorus_last_error gives a message.
+ */
+#ifndef CHORUS_H
+#define CHORUS_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CHORUS_OK 0
+#define CHORUS_EINVAL (-1) /* bad argument / order / nstages / mesh                     */
+#define CHORUS_ENOMEM (-2) /* device or host allocation failed                          */
+#define CHORUS_ECUDA (-3)  /* CUDA runtime error (message kept for chorus_last_error)   */
+#define CHORUS_ESTATE (-4) /* no state set, or a non-finite wave speed                  */
+
+typedef struct chorus_ctx chorus_ctx; /* opaque, owned by the library */
+
+/* Generic unstructured hexahedral mesh (PAPER.md:70-80 for the cubed-sphere shell; any conforming hex mesh).
+ * All pointers are HOST pointers; the arrays are copied by chorus_init. */
+typedef struct {
+  int64_t n_elem;
+  int32_t n_geom;            /* geometry nodes per direction (>= 2); tensor grid, xi fastest             */
+  const double* geom_nodes;  /* [n_geom] abscissae in [0,1], first 0, last 1 (where the map was sampled) */
+  const double* xyz;         /* [n_elem][3][n_geom^3] physical coordinates of the geometry nodes (Eq. 13) */
+  const int32_t* nbr_elem;   /* [n_elem][6] neighbour element, or -1 = inner wall, -2 = outer wall        */
+  const uint8_t* nbr_face;   /* [n_elem][6] neighbour's local face 0..5                                   */
+  const uint8_t* nbr_orient; /* [n_elem][6] orientation code (see above)                                  */
+} chorus_mesh;
+
+/* Physical parameters (Eq. 3-10; walls PAPER.md:190-198; Table 1). */
+typedef struct {
+  double gamma, R_gas, Cp;   /* Eq. 3, 4, 10                                                              */
+  double GM, Omega;          /* g = -GM r_hat / r^2; Omega along z (Eq. 5)                                */
+  double nu, kappa, eta;     /* kinematic viscosity (mu = rho nu), thermal and magnetic diffusivity       */
+  double kr_scale, kr_c[3];  /* kappa_r = kr_scale (c0 + c1 w + c2 w^2), w = r * kr_wscale */
+  double kr_wscale;
+  double c_h, a_psi;         /* GLM wave speed and damping rate (Eq. 5, 6)                                */
+  double q_bottom, T_top;    /* thermal walls (Eq. 32), used only when the flags say so     */
+  int32_t bc_mag_inner, bc_mag_outer; /* 0 perfectly conducting, 1 perfectly radial        */
+  uint32_t flags;            /* bit0 diffusion (Eq. 7), bit1 gravity, bit2 Coriolis, bit3 Powell div B sources,
+                                bit4 GLM damping, bit5 fixed-T outer wall, bit6 fixed-flux inner wall,
+                                bit7 centrifugal (off by default: not in Eq. 5)                           */
+} chorus_physics;
+
+/* Build a context: copies the mesh to the device and runs the geometry precompute (free-stream preserving
+ * curl-form metrics of the degree-n interpolant of the element map: S^d = |J| grad xi_d at the flux points,
+ * |J|, grad xi_d and x at the solution points; Eq. 13-17).
+ * order: 2..9.  cuda_stream: a cudaStream_t (NULL = default stream).  *out is NULL on failure. */
+int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chorus_physics* phys, void* cuda_stream);
+void chorus_free(chorus_ctx* ctx);
+/* Replace the physical parameters (e.g. C_h once the initial wave speed is known).  Changing kr_scale
+ * re-evaluates kappa_r at the flux points. */
+int chorus_set_physics(chorus_ctx* ctx, const chorus_physics* phys);
+
+/* q: [9][n_elem][n^3] fp64, HOST (on_device = 0) or DEVICE (on_device = 1) pointer. */
+int chorus_set_state(chorus_ctx* ctx, const double* q, int on_device);
+int chorus_get_state(chorus_ctx* ctx, double* q, int on_device);
+
+/* r = dQ/dt of the current state = -(1/|J|) div_xi F~ + M  (Eq. 16 with Eq. 5-10, 17; procedure PAPER.md:123,
+ * face treatment PAPER.md:149: BR1 common solution, averaged viscous flux, Rusanov inviscid flux).
+ * Same layout as the state.  The state is not changed. */
+int chorus_residual(chorus_ctx* ctx, double* r, int on_device);
+
+/* One time step of size dt.  nstages = 5: SSPRK(5,3) of Ruuth; 3: SSPRK(3,3); 1: forward Euler
+ * (test aids).  Each stage is a residual evaluation fused with its Runge-Kutta combination. */
+int chorus_step(chorus_ctx* ctx, double dt, int nstages);
+
+/* *out (HOST) = max over solution points of |U| + sqrt((gamma p + |B|^2)/rho): the fast magnetosonic speed
+ * maximised over direction, for the CFL condition.  Synchronises.  CHORUS_ESTATE if it is not finite. */
+int chorus_max_wavespeed(chorus_ctx* ctx, double* out);
+
+const char* chorus_last_error(const chorus_ctx* ctx);
+
+/* ---- accessors used by the parity tests and by input generation (not on the hot path) ---- */
+/* Any pointer may be NULL.  detJ [n_elem][n^3]; S [n_elem][3 fam][3 comp][n^2(n+1)]; xsol [3][n_elem][n^3];
+ * jinv [n_elem][3 d][3 p][n^3] = (grad xi_d)_p.  HOST or DEVICE pointers per on_device. */
+int chorus_get_geometry(chorus_ctx* ctx, double* detJ, double* S, double* xsol, double* jinv, int on_device);
+/* g [27][n_elem][n^3]: BR1 gradient of the current state at the solution points. */
+int chorus_get_gradient(chorus_ctx* ctx, double* g, int on_device);
+/* 1-D node sets and operators the library uses (HOST pointers, any may be NULL):
+ * xs [n], xf [n+1], Isf [(n+1)][n], Dfs [n][(n+1)]. */
+int chorus_get_operators(int order, double* xs, double* xf, double* Isf, double* Dfs);
+/* Number of kernel launches this context has enqueued since chorus_init (for bench.py's gpu_launches). */
+int64_t chorus_launch_count(const chorus_ctx* ctx);
+/* Measurement: with profiling enabled every hot-path launch is bracketed by CUDA events on the context's stream.
+ * chorus_profile_read synchronises, returns the accumulated device time (ms) and launch count per kernel class
+ * -- index 0 face-trace kernel, 1 gradient / viscous-trace kernel, 2 residual + RK kernel -- and resets them. */
+int chorus_profile(chorus_ctx* ctx, int enable);
+int chorus_profile_read(chorus_ctx* ctx, double* ms /*[3]*/, int64_t* launches /*[3]*/);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

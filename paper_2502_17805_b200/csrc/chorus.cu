@@ -1,0 +1,507 @@
+// chorus.cu -- C ABI of libchorus_b200.so (include/chorus.h): context, kernel dispatch, SSPRK driver.
+// Every step of the hot path runs in the CUDA kernels of kernels_*.cuh / geometry.cuh; this file only owns device
+// memory, marshals arguments and enqueues launches on the caller's stream.  No CPU fallback exists.
+#include "../../include/chorus.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <utility>
+#include <vector>
+
+#include "basis.h"
+#include "geometry.cuh"
+#include "kernels_residual.cuh"
+
+using namespace chorus;
+
+struct chorus_ctx {
+  int n = 0, n2 = 0, n3 = 0, nf = 0;
+  int64_t E = 0;
+  cudaStream_t stream = nullptr;
+  chorus_physics phys{};
+  PhysD ph{};
+  int num_sms = 0;
+  size_t max_smem = 0;
+  // mesh
+  int ng = 0;
+  double* d_xyz = nullptr;
+  int32_t* d_nbr_elem = nullptr;
+  uint8_t *d_nbr_face = nullptr, *d_nbr_orient = nullptr;
+  // operators for the geometry kernel
+  double *d_Gm = nullptr, *d_Dff = nullptr, *d_Efs = nullptr, *d_Dfs = nullptr;
+  // geometry
+  double *d_Sfl = nullptr, *d_detJ = nullptr, *d_jinv = nullptr, *d_xsol = nullptr, *d_krfl = nullptr;
+  // state registers (element-major) and face buffers
+  double* d_U[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  int cur = 0;
+  bool have_state = false;
+  double *d_Qf = nullptr, *d_Vf = nullptr;
+  unsigned long long* d_ws = nullptr;
+  int64_t launches = 0;
+  bool prof = false;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[3];
+  std::string err;
+};
+
+namespace {
+
+int fail(chorus_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+#define CU(c, call)                                                                                          \
+  do {                                                                                                       \
+    cudaError_t e_ = (call);                                                                                 \
+    if (e_ != cudaSuccess) return fail(c, CHORUS_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+struct ProfScope {   // brackets one launch with events when profiling is on
+  chorus_ctx* c;
+  int cls;
+  cudaEvent_t a = nullptr, b = nullptr;
+  ProfScope(chorus_ctx* c_, int cls_) : c(c_), cls(cls_) {
+    if (c->prof && cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) cudaEventRecord(a, c->stream);
+  }
+  ~ProfScope() {
+    if (a && b) {
+      cudaEventRecord(b, c->stream);
+      c->prof_ev[cls].push_back({a, b});
+    }
+  }
+};
+
+PhysD to_device_phys(const chorus_physics& p) {
+  PhysD d;
+  d.gamma = p.gamma; d.gm1 = p.gamma - 1.0; d.R = p.R_gas; d.Cp = p.Cp; d.GM = p.GM; d.Omega = p.Omega;
+  d.nu = p.nu; d.kappa = p.kappa; d.eta = p.eta; d.c_h = p.c_h; d.a_psi = p.a_psi; d.q_bottom = p.q_bottom; d.T_top = p.T_top;
+  d.bc_inner = p.bc_mag_inner; d.bc_outer = p.bc_mag_outer; d.flags = p.flags;
+  return d;
+}
+
+int grid_1d(const chorus_ctx* c, int64_t total, int block) {
+  int64_t g = (total + block - 1) / block;
+  int64_t cap = (int64_t)c->num_sms * 16;
+  return (int)(g < cap ? (g < 1 ? 1 : g) : cap);
+}
+
+// which gradient the residual kernel needs
+int gradv_of(const chorus_physics& p) { return (p.flags & kFlagDiffusion) ? 2 : (p.flags & kFlagPowell) ? 1 : 0; }
+
+template <int N>
+struct Hot {
+  using I = Ix<N>;
+  template <bool DIFF, int GRADV>
+  static int residual_launch(chorus_ctx* c, const double* Qin, const StageOut& out) {
+    constexpr size_t smem = residual_smem_bytes<N, DIFF, GRADV>();
+    if (smem > c->max_smem)
+      return fail(c, CHORUS_EINVAL, "order " + std::to_string(N) + " with these physics flags needs " + std::to_string(smem) +
+                                        " B of shared memory per CTA (limit " + std::to_string(c->max_smem) + ")");
+    auto k = residual_kernel<N, DIFF, GRADV>;
+    CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 1;
+    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, smem));
+    if (occ < 1) occ = 1;
+    const int64_t cap = (int64_t)c->num_sms * occ;
+    const int grid = (int)(c->E < cap ? c->E : cap);
+    {
+      ProfScope ps(c, 2);
+      k<<<grid, 256, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf, c->d_Vf, c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl,
+                                         c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient, out);
+    }
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    return CHORUS_OK;
+  }
+  static int trace(chorus_ctx* c, const double* Qin) {
+    constexpr size_t smem = sizeof(double) * 9 * I::n3;
+    auto k = trace_kernel<N>;
+    CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 1;
+    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, smem));
+    if (occ < 1) occ = 1;
+    const int64_t cap = (int64_t)c->num_sms * occ;
+    const int grid = (int)(c->E < cap ? c->E : cap);
+    {
+      ProfScope ps(c, 0);
+      k<<<grid, 256, smem, c->stream>>>(c->E, Qin, c->d_Qf);
+    }
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    return CHORUS_OK;
+  }
+  static int grad(chorus_ctx* c, const double* Qin, double* Vf, double* Gout) {
+    constexpr size_t smem = grad_smem_bytes<N>();
+    if (smem > c->max_smem) return fail(c, CHORUS_EINVAL, "gradient kernel: order too high for the shared-memory budget");
+    auto k = grad_kernel<N>;
+    CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 1;
+    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, smem));
+    if (occ < 1) occ = 1;
+    const int64_t cap = (int64_t)c->num_sms * occ;
+    const int grid = (int)(c->E < cap ? c->E : cap);
+    {
+      ProfScope ps(c, 1);
+      k<<<grid, 256, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf, c->d_Sfl, c->d_jinv, c->d_krfl, c->d_nbr_elem, c->d_nbr_face,
+                                         c->d_nbr_orient, Vf, Gout);
+    }
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    return CHORUS_OK;
+  }
+  // one residual evaluation of the state in Qin, fused with the output / RK combination described by `out`
+  static int stage(chorus_ctx* c, const double* Qin, const StageOut& out) {
+    int rc = trace(c, Qin);
+    if (rc) return rc;
+    const int gv = gradv_of(c->phys);
+    if (gv == 2) {
+      rc = grad(c, Qin, c->d_Vf, nullptr);
+      if (rc) return rc;
+      return residual_launch<true, 2>(c, Qin, out);
+    }
+    if (gv == 1) return residual_launch<false, 1>(c, Qin, out);
+    return residual_launch<false, 0>(c, Qin, out);
+  }
+};
+
+#define DISPATCH_N(c, expr)                                          \
+  [&]() -> int {                                                     \
+    switch ((c)->n) {                                                \
+      case 2: { using H = Hot<2>; return expr; }                     \
+      case 3: { using H = Hot<3>; return expr; }                     \
+      case 4: { using H = Hot<4>; return expr; }                     \
+      case 5: { using H = Hot<5>; return expr; }                     \
+      case 6: { using H = Hot<6>; return expr; }                     \
+      case 7: { using H = Hot<7>; return expr; }                     \
+      case 8: { using H = Hot<8>; return expr; }                     \
+      case 9: { using H = Hot<9>; return expr; }                     \
+      default: return fail((c), CHORUS_EINVAL, "order must be 2..9"); \
+    }                                                                \
+  }()
+
+int run_geometry(chorus_ctx* c) {
+  const int N1 = c->n + 1;
+  const int cap = c->ng > N1 ? c->ng : N1;
+  const size_t smem = sizeof(double) * 20 * (size_t)cap * cap * cap;
+  if (smem > c->max_smem) return fail(c, CHORUS_EINVAL, "geometry kernel: too many geometry nodes for the shared-memory budget");
+  CU(c, cudaFuncSetAttribute(geometry_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const bool need_kr = c->phys.kr_scale != 0.0;
+  if (need_kr && !c->d_krfl) CU(c, cudaMalloc(&c->d_krfl, sizeof(double) * c->E * 3 * c->nf));
+  if (!need_kr && c->d_krfl) {
+    cudaFree(c->d_krfl);
+    c->d_krfl = nullptr;
+  }
+  GeomOps op{c->d_Gm, c->d_Dff, c->d_Efs, c->d_Dfs};
+  geometry_kernel<<<(unsigned)c->E, 256, smem, c->stream>>>(c->n, c->ng, c->E, op, c->d_xyz, c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol,
+                                                            c->d_krfl, c->phys.kr_scale, c->phys.kr_c[0], c->phys.kr_c[1],
+                                                            c->phys.kr_c[2], c->phys.kr_wscale);
+  ++c->launches;
+  CU(c, cudaGetLastError());
+  return CHORUS_OK;
+}
+
+template <class T>
+int upload(chorus_ctx* c, T** dst, const T* src, size_t count) {
+  CU(c, cudaMalloc(dst, sizeof(T) * count));
+  CU(c, cudaMemcpyAsync(*dst, src, sizeof(T) * count, cudaMemcpyHostToDevice, c->stream));
+  return CHORUS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chorus_physics* phys, void* cuda_stream) {
+  if (!out) return CHORUS_EINVAL;
+  *out = nullptr;
+  if (!mesh || !phys || order < 2 || order > kMaxN || mesh->n_elem <= 0 || mesh->n_geom < 2 || mesh->n_geom > 12 || !mesh->geom_nodes ||
+      !mesh->xyz || !mesh->nbr_elem || !mesh->nbr_face || !mesh->nbr_orient)
+    return CHORUS_EINVAL;
+  for (int64_t i = 0; i < mesh->n_elem * 6; ++i) {
+    const int32_t ne = mesh->nbr_elem[i];
+    if (ne >= mesh->n_elem || ne < -2 || mesh->nbr_face[i] > 5 || mesh->nbr_orient[i] > 7) return CHORUS_EINVAL;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return CHORUS_ECUDA;   // no device: fail loudly, never fall back
+  chorus_ctx* c = new (std::nothrow) chorus_ctx;
+  if (!c) return CHORUS_ENOMEM;
+  c->n = order; c->n2 = order * order; c->n3 = c->n2 * order; c->nf = c->n2 * (order + 1);
+  c->E = mesh->n_elem;
+  c->ng = mesh->n_geom;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->phys = *phys;
+  c->ph = to_device_phys(*phys);
+  auto bail = [&](int rc) {
+    chorus_free(c);
+    return rc;
+  };
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return bail(CHORUS_ECUDA);
+  c->num_sms = prop.multiProcessorCount;
+  c->max_smem = prop.sharedMemPerBlockOptin;
+
+  // operator tables: constant memory for the hot kernels, global memory for the geometry kernel
+  Basis B = make_basis(order);
+  {
+    OpsC h;
+    std::memset(&h, 0, sizeof h);
+    std::memcpy(h.Isf, B.Isf.data(), sizeof(double) * B.Isf.size());
+    std::memcpy(h.Dfs, B.Dfs.data(), sizeof(double) * B.Dfs.size());
+    std::memcpy(h.Dss, B.Dss.data(), sizeof(double) * B.Dss.size());
+    if (cudaMemcpyToSymbolAsync(c_ops, &h, sizeof h, sizeof(OpsC) * order, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+      return bail(CHORUS_ECUDA);
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return bail(CHORUS_ECUDA);   // h is a stack object
+  }
+  std::vector<double> Gm = geometry_interp(B, mesh->geom_nodes, mesh->n_geom);
+  const size_t ng3 = (size_t)c->ng * c->ng * c->ng;
+  int rc = 0;
+  if ((rc = upload(c, &c->d_Gm, Gm.data(), Gm.size()))) return bail(rc);
+  if ((rc = upload(c, &c->d_Dff, B.Dff.data(), B.Dff.size()))) return bail(rc);
+  if ((rc = upload(c, &c->d_Efs, B.Efs.data(), B.Efs.size()))) return bail(rc);
+  if ((rc = upload(c, &c->d_Dfs, B.Dfs.data(), B.Dfs.size()))) return bail(rc);
+  if ((rc = upload(c, &c->d_xyz, mesh->xyz, (size_t)c->E * 3 * ng3))) return bail(rc);
+  if ((rc = upload(c, &c->d_nbr_elem, mesh->nbr_elem, (size_t)c->E * 6))) return bail(rc);
+  if ((rc = upload(c, &c->d_nbr_face, mesh->nbr_face, (size_t)c->E * 6))) return bail(rc);
+  if ((rc = upload(c, &c->d_nbr_orient, mesh->nbr_orient, (size_t)c->E * 6))) return bail(rc);
+  const size_t E = (size_t)c->E;
+  auto dalloc = [&](double** p, size_t count) { return cudaMalloc(p, sizeof(double) * count) == cudaSuccess; };
+  bool ok = dalloc(&c->d_Sfl, E * 9 * c->nf) && dalloc(&c->d_detJ, E * c->n3) && dalloc(&c->d_jinv, E * 9 * c->n3) &&
+            dalloc(&c->d_xsol, E * 3 * c->n3) && dalloc(&c->d_Qf, E * 54 * c->n2) && dalloc(&c->d_Vf, E * 42 * c->n2);
+  for (int k = 0; k < 5 && ok; ++k) ok = dalloc(&c->d_U[k], E * 9 * c->n3);
+  ok = ok && cudaMalloc(&c->d_ws, sizeof(unsigned long long)) == cudaSuccess;
+  if (!ok) return bail(CHORUS_ENOMEM);
+  if ((rc = run_geometry(c))) return bail(rc);
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess) return bail(CHORUS_ECUDA);   // host mesh buffers may be released by the caller
+  cudaFree(c->d_xyz);   // the geometry nodes are no longer needed unless kappa_r changes; keep a copy only on demand
+  c->d_xyz = nullptr;
+  *out = c;
+  return CHORUS_OK;
+}
+
+void chorus_free(chorus_ctx* c) {
+  if (!c) return;
+  cudaFree(c->d_xyz); cudaFree(c->d_nbr_elem); cudaFree(c->d_nbr_face); cudaFree(c->d_nbr_orient);
+  cudaFree(c->d_Gm); cudaFree(c->d_Dff); cudaFree(c->d_Efs); cudaFree(c->d_Dfs);
+  cudaFree(c->d_Sfl); cudaFree(c->d_detJ); cudaFree(c->d_jinv); cudaFree(c->d_xsol); cudaFree(c->d_krfl);
+  for (int k = 0; k < 5; ++k) cudaFree(c->d_U[k]);
+  cudaFree(c->d_Qf); cudaFree(c->d_Vf); cudaFree(c->d_ws);
+  for (auto& v : c->prof_ev)
+    for (auto& ev : v) {
+      cudaEventDestroy(ev.first);
+      cudaEventDestroy(ev.second);
+    }
+  delete c;
+}
+
+const char* chorus_last_error(const chorus_ctx* c) { return c ? c->err.c_str() : "null context"; }
+int64_t chorus_launch_count(const chorus_ctx* c) { return c ? c->launches : 0; }
+
+int chorus_set_physics(chorus_ctx* c, const chorus_physics* phys) {
+  if (!c || !phys) return CHORUS_EINVAL;
+  if (phys->kr_scale != 0.0 || c->phys.kr_scale != 0.0) {
+    const bool same = phys->kr_scale == c->phys.kr_scale && phys->kr_wscale == c->phys.kr_wscale &&
+                      std::memcmp(phys->kr_c, c->phys.kr_c, sizeof phys->kr_c) == 0;
+    if (!same) return fail(c, CHORUS_EINVAL, "kappa_r parameters are fixed at chorus_init (they are tabulated at the flux points)");
+  }
+  c->phys = *phys;
+  c->ph = to_device_phys(*phys);
+  return CHORUS_OK;
+}
+
+int chorus_set_state(chorus_ctx* c, const double* q, int on_device) {
+  if (!c || !q) return CHORUS_EINVAL;
+  const size_t count = (size_t)c->E * 9 * c->n3;
+  const double* src = q;
+  if (!on_device) {
+    CU(c, cudaMemcpyAsync(c->d_U[4], q, sizeof(double) * count, cudaMemcpyHostToDevice, c->stream));
+    src = c->d_U[4];
+  }
+  to_element_major<<<grid_1d(c, (int64_t)count, 256), 256, 0, c->stream>>>(c->E, c->n3, 9, src, c->d_U[0]);
+  ++c->launches;
+  CU(c, cudaGetLastError());
+  if (!on_device) CU(c, cudaStreamSynchronize(c->stream));
+  c->cur = 0;
+  c->have_state = true;
+  return CHORUS_OK;
+}
+
+int chorus_get_state(chorus_ctx* c, double* q, int on_device) {
+  if (!c || !q) return CHORUS_EINVAL;
+  if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
+  const size_t count = (size_t)c->E * 9 * c->n3;
+  double* dst = on_device ? q : c->d_U[(c->cur + 1) % 5];
+  from_element_major<<<grid_1d(c, (int64_t)count, 256), 256, 0, c->stream>>>(c->E, c->n3, 9, c->d_U[c->cur], dst);
+  ++c->launches;
+  CU(c, cudaGetLastError());
+  if (!on_device) {
+    CU(c, cudaMemcpyAsync(q, dst, sizeof(double) * count, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+  }
+  return CHORUS_OK;
+}
+
+int chorus_residual(chorus_ctx* c, double* r, int on_device) {
+  if (!c || !r) return CHORUS_EINVAL;
+  if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
+  const size_t count = (size_t)c->E * 9 * c->n3;
+  StageOut o{};
+  o.Rout = on_device ? r : c->d_U[(c->cur + 1) % 5];
+  const double* Qin = c->d_U[c->cur];
+  int rc = DISPATCH_N(c, H::stage(c, Qin, o));
+  if (rc) return rc;
+  if (!on_device) {
+    CU(c, cudaMemcpyAsync(r, o.Rout, sizeof(double) * count, cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+  }
+  return CHORUS_OK;
+}
+
+int chorus_step(chorus_ctx* c, double dt, int nstages) {
+  if (!c || (nstages != 1 && nstages != 3 && nstages != 5) || !(dt == dt)) return c ? fail(c, CHORUS_EINVAL, "bad dt or nstages") : CHORUS_EINVAL;
+  if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
+  int b[5];
+  for (int k = 0; k < 5; ++k) b[k] = (c->cur + k) % 5;
+  double** U = c->d_U;
+  auto run = [&](int in, int outb, const double* A0, double c0, const double* A1, double c1, const double* A2, double c2, double bdt) {
+    StageOut o{};
+    o.Qout = U[outb];
+    o.A0 = A0; o.A1 = A1; o.A2 = A2;
+    o.c0 = c0; o.c1 = c1; o.c2 = c2; o.bdt = bdt;
+    const double* Qin = U[in];
+    return DISPATCH_N(c, H::stage(c, Qin, o));
+  };
+  int rc = 0;
+  if (nstages == 1) {
+    if ((rc = run(b[0], b[1], U[b[0]], 1.0, nullptr, 0, nullptr, 0, dt))) return rc;
+    c->cur = b[1];
+  } else if (nstages == 3) {   // Shu-Osher SSPRK(3,3)
+    if ((rc = run(b[0], b[1], U[b[0]], 1.0, nullptr, 0, nullptr, 0, dt))) return rc;
+    if ((rc = run(b[1], b[2], U[b[0]], 0.75, U[b[1]], 0.25, nullptr, 0, 0.25 * dt))) return rc;
+    if ((rc = run(b[2], b[3], U[b[0]], 1.0 / 3.0, U[b[2]], 2.0 / 3.0, nullptr, 0, (2.0 / 3.0) * dt))) return rc;
+    c->cur = b[3];
+  } else {
+    // SSPRK(5,3) of Ruuth in Shu-Osher form; F(u0) and F(u1) of stages 4 and 5 are eliminated through
+    // dt F(u0) = (u1 - u0)/beta1 and dt F(u1) = (u2 - u1)/beta1, so only state registers are kept.
+    const double be1 = 0.37726891511710;
+    const double a30 = 0.56656131914033, a32 = 0.43343868085967, b32 = 0.16352294089771;
+    const double a40 = 0.09299483444413, a41 = 0.00002090369620, a43 = 0.90698426185967, b40 = 0.00071997378654, b43 = 0.34217696850008;
+    const double a50 = 0.00736132260920, a51 = 0.20127980325145, a52 = 0.00182955389682, a54 = 0.78952932024253;
+    const double b50 = 0.00277719819460, b51 = 0.00001567934613, b54 = 0.29786487010104;
+    const double c40 = a40 - b40 / be1, c41 = a41 + b40 / be1;
+    const double c50 = a50 - b50 / be1, c51 = a51 + b50 / be1 - b51 / be1, c52 = a52 + b51 / be1;
+    (void)c50;   // = -4e-16: u0's weight in stage 5 cancels to round-off and is dropped
+    if ((rc = run(b[0], b[1], U[b[0]], 1.0, nullptr, 0, nullptr, 0, be1 * dt))) return rc;
+    if ((rc = run(b[1], b[2], U[b[1]], 1.0, nullptr, 0, nullptr, 0, be1 * dt))) return rc;
+    if ((rc = run(b[2], b[3], U[b[0]], a30, U[b[2]], a32, nullptr, 0, b32 * dt))) return rc;
+    if ((rc = run(b[3], b[4], U[b[0]], c40, U[b[1]], c41, U[b[3]], a43, b43 * dt))) return rc;
+    if ((rc = run(b[4], b[0], U[b[1]], c51, U[b[2]], c52, U[b[4]], a54, b54 * dt))) return rc;
+    c->cur = b[0];
+  }
+  return CHORUS_OK;
+}
+
+int chorus_max_wavespeed(chorus_ctx* c, double* out) {
+  if (!c || !out) return CHORUS_EINVAL;
+  if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
+  CU(c, cudaMemsetAsync(c->d_ws, 0, sizeof(unsigned long long), c->stream));
+  const int64_t total = c->E * c->n3;
+  int grid = grid_1d(c, total, 256);
+  wavespeed_kernel<<<grid, 256, 0, c->stream>>>(c->E, c->n3, c->ph, c->d_U[c->cur], c->d_ws);
+  ++c->launches;
+  CU(c, cudaGetLastError());
+  unsigned long long bits = 0;
+  CU(c, cudaMemcpyAsync(&bits, c->d_ws, sizeof bits, cudaMemcpyDeviceToHost, c->stream));
+  CU(c, cudaStreamSynchronize(c->stream));
+  double v;
+  std::memcpy(&v, &bits, sizeof v);
+  *out = v;
+  if (!std::isfinite(v)) return fail(c, CHORUS_ESTATE, "non-finite wave speed");
+  return CHORUS_OK;
+}
+
+int chorus_get_geometry(chorus_ctx* c, double* detJ, double* S, double* xsol, double* jinv, int on_device) {
+  if (!c) return CHORUS_EINVAL;
+  const size_t E = (size_t)c->E;
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  if (detJ) CU(c, cudaMemcpyAsync(detJ, c->d_detJ, sizeof(double) * E * c->n3, kind, c->stream));
+  if (S) CU(c, cudaMemcpyAsync(S, c->d_Sfl, sizeof(double) * E * 9 * c->nf, kind, c->stream));
+  if (jinv) CU(c, cudaMemcpyAsync(jinv, c->d_jinv, sizeof(double) * E * 9 * c->n3, kind, c->stream));
+  if (xsol) {
+    const size_t count = E * 3 * c->n3;
+    double* dst = on_device ? xsol : c->d_U[(c->cur + 1) % 5];
+    from_element_major<<<grid_1d(c, (int64_t)count, 256), 256, 0, c->stream>>>(c->E, c->n3, 3, c->d_xsol, dst);
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    if (!on_device) CU(c, cudaMemcpyAsync(xsol, dst, sizeof(double) * count, cudaMemcpyDeviceToHost, c->stream));
+  }
+  if (!on_device) CU(c, cudaStreamSynchronize(c->stream));
+  return CHORUS_OK;
+}
+
+int chorus_get_gradient(chorus_ctx* c, double* g, int on_device) {
+  if (!c || !g) return CHORUS_EINVAL;
+  if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
+  const size_t count = (size_t)c->E * 27 * c->n3;
+  double *tmp = nullptr, *tmp2 = nullptr;
+  CU(c, cudaMalloc(&tmp, sizeof(double) * count));
+  if (!on_device && cudaMalloc(&tmp2, sizeof(double) * count) != cudaSuccess) {
+    cudaFree(tmp);
+    return fail(c, CHORUS_ENOMEM, "gradient scratch");
+  }
+  const double* Qin = c->d_U[c->cur];
+  int rc = DISPATCH_N(c, H::trace(c, Qin));
+  if (!rc) rc = DISPATCH_N(c, H::grad(c, Qin, nullptr, tmp));
+  if (!rc) {
+    double* dst = on_device ? g : tmp2;
+    from_element_major<<<grid_1d(c, (int64_t)count, 256), 256, 0, c->stream>>>(c->E, c->n3, 27, tmp, dst);
+    ++c->launches;
+    if (cudaGetLastError() != cudaSuccess) rc = fail(c, CHORUS_ECUDA, "from_element_major launch");
+    if (!rc && !on_device && cudaMemcpyAsync(g, dst, sizeof(double) * count, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+      rc = fail(c, CHORUS_ECUDA, "gradient copy");
+  }
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess && !rc) rc = fail(c, CHORUS_ECUDA, "stream sync");
+  cudaFree(tmp);
+  cudaFree(tmp2);
+  return rc;
+}
+
+int chorus_profile(chorus_ctx* c, int enable) {
+  if (!c) return CHORUS_EINVAL;
+  c->prof = enable != 0;
+  return CHORUS_OK;
+}
+
+int chorus_profile_read(chorus_ctx* c, double* ms, int64_t* launches) {
+  if (!c || !ms || !launches) return CHORUS_EINVAL;
+  CU(c, cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < 3; ++k) {
+    double tot = 0.0;
+    for (auto& ev : c->prof_ev[k]) {
+      float t = 0.f;
+      cudaEventElapsedTime(&t, ev.first, ev.second);
+      tot += t;
+      cudaEventDestroy(ev.first);
+      cudaEventDestroy(ev.second);
+    }
+    ms[k] = tot;
+    launches[k] = (int64_t)c->prof_ev[k].size();
+    c->prof_ev[k].clear();
+  }
+  return CHORUS_OK;
+}
+
+int chorus_get_operators(int order, double* xs, double* xf, double* Isf, double* Dfs) {
+  if (order < 2 || order > kMaxN) return CHORUS_EINVAL;
+  Basis B = make_basis(order);
+  if (xs) std::memcpy(xs, B.xs.data(), sizeof(double) * B.xs.size());
+  if (xf) std::memcpy(xf, B.xf.data(), sizeof(double) * B.xf.size());
+  if (Isf) std::memcpy(Isf, B.Isf.data(), sizeof(double) * B.Isf.size());
+  if (Dfs) std::memcpy(Dfs, B.Dfs.data(), sizeof(double) * B.Dfs.size());
+  return CHORUS_OK;
+}
+
+}  // extern "C"

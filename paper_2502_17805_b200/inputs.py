@@ -395,3 +395,58 @@ def workload(name: str) -> Workload:
         "sweep_n9": Workload("sweep_n9", 9, 18, 7, 3.0, 4, 1e-3, True, 2, sh3),
     }
     return table[name]
+
+
+# --------------------------------------------------------------------------------------
+# a walled box whose elements have randomly rotated local axes: exercises every face pairing
+# (xi<->eta<->zeta) and every orientation code; test input only
+# --------------------------------------------------------------------------------------
+def _proper_rotations():
+    rots = []
+    for perm in itertools.permutations(range(3)):
+        for flips in itertools.product((False, True), repeat=3):
+            sign = 1
+            p = list(perm)                      # parity of the permutation
+            for i in range(3):
+                for j in range(i + 1, 3):
+                    if p[i] > p[j]:
+                        sign = -sign
+            for f in flips:
+                if f:
+                    sign = -sign
+            if sign > 0:
+                rots.append((perm, flips))
+    return rots
+
+
+def scrambled_box(nx: int, ny: int, nz: int, lengths, gnodes: np.ndarray, seed: int, distort: float = 0.0):
+    """nx*ny*nz hexes on a box with walls on every outer face (z-low faces tagged -1, all others -2); every
+    element's local (xi,eta,zeta) axes are rotated by a random proper rotation, so neighbours meet through
+    arbitrary local faces and orientations.  gnodes must be symmetric under x -> 1-x."""
+    g = np.asarray(gnodes, np.float64)
+    if np.abs(g + g[::-1] - 1.0).max() > 1e-14:
+        raise ValueError("gnodes must be symmetric")
+    base = periodic_box(nx, ny, nz, lengths, g, distort=distort, walls_z=True)
+    ng, E = g.size, base["n_elem"]
+    xyz = base["xyz"].reshape(E, 3, ng, ng, ng)          # [E,comp,c,b,a]
+    rng = np.random.Generator(np.random.PCG64(seed))
+    rots = _proper_rotations()
+    out = np.empty_like(xyz)
+    for e in range(E):
+        perm, flips = rots[rng.integers(len(rots))]
+        A = np.transpose(xyz[e], (0, 3, 2, 1))             # [comp,a,b,c] = axes (xi,eta,zeta)
+        A = np.transpose(A, (0,) + tuple(1 + p for p in perm))
+        for ax, f in enumerate(flips):
+            if f:
+                A = np.flip(A, axis=1 + ax)
+        out[e] = np.transpose(A, (0, 3, 2, 1))             # back to [comp,c,b,a]
+    corners = np.transpose(out[:, :, ::ng - 1, ::ng - 1, ::ng - 1], (0, 1, 4, 3, 2))   # [E,3,xi,eta,zeta]
+    Lz = lengths[2]
+
+    def wall_tag(c):
+        return np.where(c[:, 2] < 1e-9 * Lz, -1, -2).astype(np.int32)
+
+    nbr_elem, nbr_face, nbr_orient = hex_connectivity(corners, wall_tag)
+    return dict(n_elem=E, n_geom=ng, geom_nodes=g.copy(), xyz=np.ascontiguousarray(out.reshape(E, 3, ng ** 3)),
+                nbr_elem=nbr_elem, nbr_face=nbr_face, nbr_orient=nbr_orient, kind="scrambled_box",
+                lengths=tuple(lengths), shape=(nx, ny, nz))

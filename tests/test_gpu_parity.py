@@ -1,0 +1,213 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; norms of DESIGN.md readings G24 / G25):
+  residual   max |dR_c| / max A_c  <= 1e-12   (A = the oracle's magnitude residual)
+  state      max |dQ_c| / max |Q_c| <= 1e-9    after 10 RK steps
+  geometry   <= 1e-12 relative to the array's max (fp64 curl-form metrics; see test_p16 for the floor)
+"""
+import numpy as np
+import pytest
+
+import paper_2502_17805_b200 as P
+from paper_2502_17805_b200 import inputs as I
+from oracle import binding as ob
+from helpers import g24_error, g25_error
+
+pytestmark = pytest.mark.gpu
+
+RES_TOL = 1e-12
+STATE_TOL = 1e-9
+GEO_TOL = 1e-12
+
+
+def shell_case(n, nz, nr, N_rho, seed, diff, dipole=True, u_amp=1e-4, b_amp=1e-3, flatten=0.0, extra_flags=0, **phys_kw):
+    sh = I.Shell(N_rho=N_rho)
+    w = I.Workload("case", n, nz, nr, N_rho, seed, diff, dipole, shell=sh)
+    mesh = w.mesh()
+    o = ob.Oracle(mesh, n, I.Physics())
+    xs = o.geometry()["xsol"]
+    Q = I.shell_state(xs, sh, seed, u_amp=u_amp, b_amp=b_amp, dipole=dipole, flatten=flatten)
+    o.set_state(Q)
+    c_h = o.max_wavespeed()
+    phys = w.physics(c_h)
+    if extra_flags or phys_kw:
+        phys = phys.copy(flags=phys.flags | extra_flags, **phys_kw)
+    o.set_physics(phys)
+    g = P.Chorus(mesh, n, phys)
+    g.set_state(Q)
+    return w, mesh, o, g, Q, phys
+
+
+def check_residual(o, g, tol=RES_TOL):
+    r_ref, a_ref = o.residual(True)
+    r = g.residual()
+    err = g24_error(r, r_ref, a_ref)
+    assert np.isfinite(r).all()
+    assert err.max() <= tol, err
+    return err
+
+
+def test_geometry_parity_shell_and_box():
+    for mesh, n in ((I.cubed_sphere_shell(4, 2, 0.7, 0.95, I.lobatto_abscissae(7)), 6),
+                    (I.scrambled_box(2, 2, 2, (1.0, 1.1, 0.9), I.lobatto_abscissae(5), seed=2, distort=0.1), 4),
+                    (I.cubed_sphere_shell(2, 1, 0.7, 0.95, I.lobatto_abscissae(4)), 7)):
+        go = ob.Oracle(mesh, n, I.Physics()).geometry()
+        gg = P.Chorus(mesh, n, I.Physics()).geometry()
+        for k in ("detJ", "S", "xsol", "jinv"):
+            assert np.abs(gg[k] - go[k]).max() <= GEO_TOL * np.abs(go[k]).max(), k
+
+
+def test_config0_residual_gradient_wavespeed_parity():
+    """BASELINE config 0: 6x4x4x2 shell, n = 6, N_rho = 1, gravity + Coriolis + GLM, diffusion off."""
+    w, mesh, o, g, Q, phys = shell_case(6, 4, 2, 1.0, 0, 0.0)
+    assert mesh["n_elem"] == 192
+    check_residual(o, g)
+    assert abs(g.max_wavespeed() / o.max_wavespeed() - 1) < 1e-14
+    np.testing.assert_array_equal(g.get_state(), Q)               # set/get round trip is exact
+    G_ref = o.gradient()
+    G = g.gradient()
+    assert np.abs(G - G_ref).max() <= 1e-12 * np.abs(G_ref).max()
+
+
+def test_config0_ten_rk_stages_and_ten_steps():
+    w, mesh, o, g, Q, phys = shell_case(6, 4, 2, 1.0, 0, 0.0)
+    _, xf, _, _ = P.get_operators(6)
+    dt = w.dt(o.max_wavespeed(), xf[1] - xf[0])
+    for _ in range(2):                                             # "10 RK stages" = 2 steps of SSPRK(5,3)
+        o.step(dt, 5); g.step(dt, 5)
+    assert g25_error(g.get_state(), o.get_state(), phys.c_h).max() <= STATE_TOL
+    for _ in range(8):                                             # ... and the 10-step state check of north_star
+        o.step(dt, 5); g.step(dt, 5)
+    q = g.get_state()
+    err = g25_error(q, o.get_state(), phys.c_h)
+    assert np.isfinite(q).all() and err.max() <= STATE_TOL, err
+    assert np.abs(q - Q).max() > 1e-9                              # the state did move
+    check_residual(o, g)
+
+
+def test_full_physics_shell_parity():
+    """Config-1 physics (N_rho = 3, nu = kappa = eta = 1e-3, all terms) on a 6x4x4x3 shell."""
+    w, mesh, o, g, Q, phys = shell_case(6, 4, 3, 3.0, 1, 1e-3)
+    check_residual(o, g)
+    _, xf, _, _ = P.get_operators(6)
+    for _ in range(10):
+        dt = w.dt(o.max_wavespeed(), xf[1] - xf[0])
+        assert abs(g.max_wavespeed() / o.max_wavespeed() - 1) < 1e-12
+        o.step(dt, 5); g.step(dt, 5)
+    err = g25_error(g.get_state(), o.get_state(), phys.c_h)
+    assert err.max() <= STATE_TOL, err
+    check_residual(o, g)
+
+
+def test_nonequilibrium_input_naive_relative_error():
+    """Reading G24, second half: on a non-equilibrium input (perturbations x1000, background flattened) the plain
+    relative error max|dR_c| / max|R_c| is itself <= 1e-12 for the variables that evolve."""
+    w, mesh, o, g, Q, phys = shell_case(6, 4, 2, 3.0, 5, 1e-3, u_amp=0.1, b_amp=1.0, flatten=0.7)
+    r_ref, a_ref = o.residual(True)
+    r = g.residual()
+    naive = np.abs(r - r_ref).reshape(9, -1).max(1) / np.abs(r_ref).reshape(9, -1).max(1)
+    assert naive.max() <= 1e-12, naive
+    assert g24_error(r, r_ref, a_ref).max() <= RES_TOL
+
+
+@pytest.mark.parametrize("wall_opts", [dict(bc_mag_inner=I.BC_RADIAL, bc_mag_outer=I.BC_CONDUCTING),
+                                       dict(T_top=0.05, q_bottom=0.02, extra_flags=I.FLAG_FIXED_T_OUTER | I.FLAG_FIXED_FLUX_INNER),
+                                       dict(extra_flags=I.FLAG_CENTRIFUGAL),
+                                       dict(kr_scale=2e-3, kr_c=(1.0, -0.5, 0.25), kr_wscale=1.3)])
+def test_wall_and_option_variants_parity(wall_opts):
+    kw = dict(wall_opts)
+    extra = kw.pop("extra_flags", 0)
+    w, mesh, o, g, Q, phys = shell_case(5, 3, 2, 3.0, 7, 2e-3, u_amp=0.01, b_amp=0.05, extra_flags=extra, **kw)
+    check_residual(o, g)
+
+
+def test_all_orientation_codes_parity():
+    n = 4
+    mesh = I.scrambled_box(3, 3, 3, (1.0, 1.1, 0.9), I.lobatto_abscissae(n + 1), seed=5, distort=0.1)
+    for flags in (I.FLAG_POWELL, I.FLAG_POWELL | I.FLAG_DIFFUSION):
+        phys = I.Physics(c_h=1.2, nu=0.01, kappa=0.02, eta=0.015, flags=flags)
+        o = ob.Oracle(mesh, n, phys)
+        g = P.Chorus(mesh, n, phys)
+        x = o.geometry()["xsol"]
+        rng = np.random.default_rng(3)
+        sh = x.shape[1:]
+        Q = I.conserved(1 + 0.2 * np.sin(3 * x[0]) + 0.05 * rng.uniform(-1, 1, sh), 0.2 * rng.uniform(-1, 1, (3,) + sh) + 0.1,
+                        1 + 0.1 * np.cos(2 * x[1]), 0.3 * rng.uniform(-1, 1, (3,) + sh) + 0.2, 0.1 * rng.uniform(-1, 1, sh), 5 / 3)
+        o.set_state(Q); g.set_state(Q)
+        check_residual(o, g)
+        # free stream on the GPU: uniform static state is preserved to round-off through every orientation
+        Q[:] = I.conserved(1.2, np.zeros(3), 1.5, np.zeros(3), np.float64(0.0), 5 / 3)[:, None, None]
+        o.set_state(Q); g.set_state(Q)
+        _, a = o.residual(True)
+        assert np.abs(g.residual()).max() <= 1e-13 * a.max()
+
+
+@pytest.mark.parametrize("n,diff", [(2, 1e-3), (3, 1e-3), (4, 1e-3), (5, 1e-3), (6, 1e-3), (7, 0.0), (8, 0.0)])
+def test_order_sweep_parity(n, diff):
+    """BASELINE config 4 (order sweep), at sizes the oracle finishes in seconds."""
+    w, mesh, o, g, Q, phys = shell_case(n, 3, 2, 3.0, 4, diff)
+    check_residual(o, g)
+    _, xf, _, _ = P.get_operators(n)
+    dt = w.dt(o.max_wavespeed(), xf[1] - xf[0])
+    for _ in range(2):
+        o.step(dt, 5); g.step(dt, 5)
+    assert g25_error(g.get_state(), o.get_state(), phys.c_h).max() <= STATE_TOL
+
+
+@pytest.mark.parametrize("nstages", [1, 3])
+def test_other_rk_schemes_parity(nstages):
+    w, mesh, o, g, Q, phys = shell_case(4, 3, 2, 1.0, 9, 1e-3)
+    _, xf, _, _ = P.get_operators(4)
+    dt = 0.5 * w.dt(o.max_wavespeed(), xf[1] - xf[0])
+    for _ in range(3):
+        o.step(dt, nstages); g.step(dt, nstages)
+    assert g25_error(g.get_state(), o.get_state(), phys.c_h).max() <= STATE_TOL
+
+
+def test_device_pointers_and_streams():
+    import torch
+    w, mesh, o, g, Q, phys = shell_case(4, 3, 2, 1.0, 9, 1e-3)
+    qd = torch.from_numpy(Q).cuda()
+    g.set_state(qd)
+    r_dev = g.residual(device=True)
+    r_host = g.residual()
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(r_dev.cpu().numpy(), r_host)
+    np.testing.assert_array_equal(g.get_state(device=True).cpu().numpy(), Q)
+    n0 = g.launch_count()
+    g.step(1e-4, 5)
+    assert g.launch_count() - n0 == 15            # trace + gradient + residual per stage
+
+
+def test_error_paths():
+    mesh = I.periodic_box(2, 1, 1, (1, 1, 1), I.lobatto_abscissae(4))
+    g = P.Chorus(mesh, 3, I.Physics(c_h=1.0))
+    with pytest.raises(P.ChorusError) as ei:
+        g.residual()
+    assert ei.value.code == -4                    # CHORUS_ESTATE: no state set
+    with pytest.raises(P.ChorusError):
+        g.step(1e-3, 4)                           # unsupported stage count
+    with pytest.raises(P.ChorusError):
+        P.Chorus(mesh, 10, I.Physics())
+    bad = dict(mesh); bad["nbr_elem"] = mesh["nbr_elem"].copy(); bad["nbr_elem"][0, 0] = 99
+    with pytest.raises(P.ChorusError):
+        P.Chorus(bad, 3, I.Physics())
+    Q = np.zeros(g.shape); Q[0] = 1.0; Q[4] = np.nan
+    g.set_state(Q)
+    with pytest.raises(P.ChorusError) as ei:
+        g.max_wavespeed()
+    assert ei.value.code == -4                    # non-finite wave speed
+
+
+def test_empty_and_single_element_edge_cases():
+    mesh = I.periodic_box(1, 1, 1, (1, 1, 1), I.lobatto_abscissae(3))       # one element, its own neighbour
+    phys = I.Physics(c_h=1.0, nu=0.01, kappa=0.01, eta=0.01, flags=I.FLAG_DIFFUSION | I.FLAG_POWELL)
+    o, g = ob.Oracle(mesh, 3, phys), P.Chorus(mesh, 3, phys)
+    x = o.geometry()["xsol"]
+    Q = I.conserved(1 + 0.1 * np.sin(2 * np.pi * x[0]), 0.1 * np.stack([np.cos(2 * np.pi * x[1])] * 3), 1 + 0 * x[0],
+                    0.2 * np.stack([np.sin(2 * np.pi * x[2])] * 3), 0 * x[0], 5 / 3)
+    o.set_state(Q); g.set_state(Q)
+    check_residual(o, g)
+    empty = dict(mesh); empty["n_elem"] = 0
+    with pytest.raises(P.ChorusError):
+        P.Chorus(empty, 3, phys)

@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libchorus_b200.so")
+LIB_PATH = os.environ.get("CHORUS_LIB", os.path.join(HERE, "libchorus_b200.so"))   # override: A/B testing of builds
 
 CHORUS_OK, CHORUS_EINVAL, CHORUS_ENOMEM, CHORUS_ECUDA, CHORUS_ESTATE = 0, -1, -2, -3, -4
 

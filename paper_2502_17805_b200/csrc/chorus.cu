@@ -7,6 +7,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <utility>
@@ -14,7 +15,7 @@
 
 #include "basis.h"
 #include "geometry.cuh"
-#include "kernels_residual.cuh"
+#include "kernels_mma.cuh"
 
 using namespace chorus;
 
@@ -42,6 +43,7 @@ struct chorus_ctx {
   double *d_Qf = nullptr, *d_Vf = nullptr;
   unsigned long long* d_ws = nullptr;
   int64_t launches = 0;
+  bool use_mma = true;   // orders 4..7: DMMA chain kernel (CHORUS_KERNELS=scalar selects the shared-memory pencil kernel)
   bool prof = false;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[3];
   std::string err;
@@ -116,6 +118,31 @@ struct Hot {
     CU(c, cudaGetLastError());
     return CHORUS_OK;
   }
+  template <bool DIFF, int GRADV>
+  static int residual_mma_launch(chorus_ctx* c, const double* Qin, const StageOut& out) {
+    if constexpr (N >= 4 && N <= 7) {
+      constexpr size_t smem = residual_mma_smem_bytes<N, GRADV>();
+      constexpr int threads = Mma<N>::kThreads;
+      auto k = residual_mma_kernel<N, DIFF, GRADV>;
+      CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      CU(c, cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+      int occ = 1;
+      CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, threads, smem));
+      if (occ < 1) occ = 1;
+      const int64_t cap = (int64_t)c->num_sms * occ;
+      const int grid = (int)(c->E < cap ? c->E : cap);
+      {
+        ProfScope ps(c, 2);
+        k<<<grid, threads, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf, c->d_Vf, c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl,
+                                               c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient, out);
+      }
+      ++c->launches;
+      CU(c, cudaGetLastError());
+      return CHORUS_OK;
+    } else {
+      return residual_launch<DIFF, GRADV>(c, Qin, out);
+    }
+  }
   static int trace(chorus_ctx* c, const double* Qin) {
     constexpr size_t smem = sizeof(double) * 9 * I::n3;
     auto k = trace_kernel<N>;
@@ -160,10 +187,10 @@ struct Hot {
     if (gv == 2) {
       rc = grad(c, Qin, c->d_Vf, nullptr);
       if (rc) return rc;
-      return residual_launch<true, 2>(c, Qin, out);
+      return c->use_mma ? residual_mma_launch<true, 2>(c, Qin, out) : residual_launch<true, 2>(c, Qin, out);
     }
-    if (gv == 1) return residual_launch<false, 1>(c, Qin, out);
-    return residual_launch<false, 0>(c, Qin, out);
+    if (gv == 1) return c->use_mma ? residual_mma_launch<false, 1>(c, Qin, out) : residual_launch<false, 1>(c, Qin, out);
+    return c->use_mma ? residual_mma_launch<false, 0>(c, Qin, out) : residual_launch<false, 0>(c, Qin, out);
   }
 };
 
@@ -241,6 +268,7 @@ int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chor
   int dev = 0;
   cudaDeviceProp prop;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return bail(CHORUS_ECUDA);
+  if (const char* kv = std::getenv("CHORUS_KERNELS")) c->use_mma = std::strcmp(kv, "scalar") != 0;
   c->num_sms = prop.multiProcessorCount;
   c->max_smem = prop.sharedMemPerBlockOptin;
 

@@ -15,7 +15,7 @@
 
 #include "basis.h"
 #include "geometry.cuh"
-#include "kernels_mma.cuh"
+#include "kernels_stage.cuh"
 
 using namespace chorus;
 
@@ -40,10 +40,14 @@ struct chorus_ctx {
   double* d_U[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   int cur = 0;
   bool have_state = false;
-  double *d_Qf = nullptr, *d_Vf = nullptr;
+  double* d_Qf[2] = {nullptr, nullptr};   // face traces, double-buffered: a stage reads one and emits the next state's into the other
+  int qf_cur = 0;                         // which buffer holds the traces of the current state ...
+  bool traces_valid = false;              // ... if any does
+  double* d_Vf = nullptr;
   unsigned long long* d_ws = nullptr;
   int64_t launches = 0;
-  bool use_mma = true;   // orders 4..7: DMMA chain kernel (CHORUS_KERNELS=scalar selects the shared-memory pencil kernel)
+  bool use_mma = true;   // orders 4..7: two-kernel DMMA pipeline (kernels_stage.cuh); CHORUS_KERNELS=scalar selects the
+                         // three-kernel shared-memory path that serves the other orders (kernels_residual.cuh)
   bool prof = false;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[3];
   std::string err;
@@ -111,19 +115,20 @@ struct Hot {
     const int grid = (int)(c->E < cap ? c->E : cap);
     {
       ProfScope ps(c, 2);
-      k<<<grid, 256, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf, c->d_Vf, c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl,
+      k<<<grid, 256, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf[0], c->d_Vf, c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl,
                                          c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient, out);
     }
     ++c->launches;
     CU(c, cudaGetLastError());
     return CHORUS_OK;
   }
+  // ---- production pipeline (orders 4..7): main kernel, then (diffusion) the face kernel
   template <bool DIFF, int GRADV>
-  static int residual_mma_launch(chorus_ctx* c, const double* Qin, const StageOut& out) {
+  static int main_launch(chorus_ctx* c, const StageIO& io) {
     if constexpr (N >= 4 && N <= 7) {
-      constexpr size_t smem = residual_mma_smem_bytes<N, GRADV>();
+      constexpr size_t smem = stage_main_smem_bytes<N, GRADV>();
       constexpr int threads = Mma<N>::kThreads;
-      auto k = residual_mma_kernel<N, DIFF, GRADV>;
+      auto k = stage_main_kernel<N, DIFF, GRADV>;
       CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       CU(c, cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
       int occ = 1;
@@ -133,17 +138,54 @@ struct Hot {
       const int grid = (int)(c->E < cap ? c->E : cap);
       {
         ProfScope ps(c, 2);
-        k<<<grid, threads, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf, c->d_Vf, c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl,
-                                               c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient, out);
+        k<<<grid, threads, smem, c->stream>>>(c->E, c->ph, io, geo(c));
       }
       ++c->launches;
       CU(c, cudaGetLastError());
       return CHORUS_OK;
     } else {
-      return residual_launch<DIFF, GRADV>(c, Qin, out);
+      return fail(c, CHORUS_EINVAL, "the DMMA pipeline serves orders 4..7");
     }
   }
-  static int trace(chorus_ctx* c, const double* Qin) {
+  static int face_launch(chorus_ctx* c, const StageIO& io) {
+    constexpr size_t smem = stage_face_smem_bytes<N>();
+    auto k = stage_face_kernel<N>;
+    CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 1;
+    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, smem));
+    if (occ < 1) occ = 1;
+    const int64_t cap = (int64_t)c->num_sms * occ;
+    const int grid = (int)(c->E < cap ? c->E : cap);
+    {
+      ProfScope ps(c, 1);
+      k<<<grid, 256, smem, c->stream>>>(c->E, io, geo(c));
+    }
+    ++c->launches;
+    CU(c, cudaGetLastError());
+    return CHORUS_OK;
+  }
+  static Geo geo(const chorus_ctx* c) {
+    return Geo{c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl, c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient};
+  }
+  // one residual evaluation through the pipeline.  io carries Qe and the outputs; the traces of Qe must be in d_Qf[qf_cur].
+  static int stage_pipeline(chorus_ctx* c, StageIO io) {
+    io.Qf = c->d_Qf[c->qf_cur];
+    io.QfOut = c->d_Qf[c->qf_cur ^ 1];
+    io.Vf = c->d_Vf;
+    const int gv = gradv_of(c->phys);
+    int rc;
+    if (gv == 2) {
+      if ((rc = main_launch<true, 2>(c, io))) return rc;
+      rc = face_launch(c, io);
+    } else if (gv == 1) {
+      rc = main_launch<false, 1>(c, io);
+    } else {
+      rc = main_launch<false, 0>(c, io);
+    }
+    if (!rc && io.Qout != nullptr) c->qf_cur ^= 1;   // the traces of the new state were emitted into the other buffer
+    return rc;
+  }
+  static int trace(chorus_ctx* c, const double* Qin, double* Qf) {
     constexpr size_t smem = sizeof(double) * 9 * I::n3;
     auto k = trace_kernel<N>;
     CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -154,7 +196,7 @@ struct Hot {
     const int grid = (int)(c->E < cap ? c->E : cap);
     {
       ProfScope ps(c, 0);
-      k<<<grid, 256, smem, c->stream>>>(c->E, Qin, c->d_Qf);
+      k<<<grid, 256, smem, c->stream>>>(c->E, Qin, Qf);
     }
     ++c->launches;
     CU(c, cudaGetLastError());
@@ -172,25 +214,45 @@ struct Hot {
     const int grid = (int)(c->E < cap ? c->E : cap);
     {
       ProfScope ps(c, 1);
-      k<<<grid, 256, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf, c->d_Sfl, c->d_jinv, c->d_krfl, c->d_nbr_elem, c->d_nbr_face,
+      k<<<grid, 256, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf[0], c->d_Sfl, c->d_jinv, c->d_krfl, c->d_nbr_elem, c->d_nbr_face,
                                          c->d_nbr_orient, Vf, Gout);
     }
     ++c->launches;
     CU(c, cudaGetLastError());
     return CHORUS_OK;
   }
-  // one residual evaluation of the state in Qin, fused with the output / RK combination described by `out`
-  static int stage(chorus_ctx* c, const double* Qin, const StageOut& out) {
-    int rc = trace(c, Qin);
+  // legacy three-kernel path (orders 2, 3, 8, 9 and CHORUS_KERNELS=scalar): trace, gradient, residual + RK
+  static int stage_legacy(chorus_ctx* c, const double* Qin, const StageOut& out) {
+    c->traces_valid = false;   // d_Qf[0] is this path's scratch
+    c->qf_cur = 0;
+    int rc = trace(c, Qin, c->d_Qf[0]);
     if (rc) return rc;
     const int gv = gradv_of(c->phys);
     if (gv == 2) {
       rc = grad(c, Qin, c->d_Vf, nullptr);
       if (rc) return rc;
-      return c->use_mma ? residual_mma_launch<true, 2>(c, Qin, out) : residual_launch<true, 2>(c, Qin, out);
+      return residual_launch<true, 2>(c, Qin, out);
     }
-    if (gv == 1) return c->use_mma ? residual_mma_launch<false, 1>(c, Qin, out) : residual_launch<false, 1>(c, Qin, out);
-    return c->use_mma ? residual_mma_launch<false, 0>(c, Qin, out) : residual_launch<false, 0>(c, Qin, out);
+    if (gv == 1) return residual_launch<false, 1>(c, Qin, out);
+    return residual_launch<false, 0>(c, Qin, out);
+  }
+  // one residual evaluation of the state in Qin, fused with the output / RK combination described by `out`.
+  // scratch: a state-sized buffer distinct from Qin, the outputs and the stage registers (residual mode with diffusion).
+  static int stage(chorus_ctx* c, const double* Qin, const StageOut& out, double* scratch) {
+    if (!(c->use_mma && N >= 4 && N <= 7)) return stage_legacy(c, Qin, out);
+    if (!c->traces_valid) {
+      int rc = trace(c, Qin, c->d_Qf[c->qf_cur]);
+      if (rc) return rc;
+      c->traces_valid = true;
+    }
+    StageIO io{};
+    io.Qe = Qin;
+    io.Rout = out.Rout;
+    io.Qout = out.Qout;
+    io.Part = out.Qout ? out.Qout : scratch;
+    io.A0 = out.A0; io.A1 = out.A1; io.A2 = out.A2;
+    io.c0 = out.c0; io.c1 = out.c1; io.c2 = out.c2; io.bdt = out.bdt;
+    return stage_pipeline(c, io);
   }
 };
 
@@ -298,7 +360,8 @@ int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chor
   const size_t E = (size_t)c->E;
   auto dalloc = [&](double** p, size_t count) { return cudaMalloc(p, sizeof(double) * count) == cudaSuccess; };
   bool ok = dalloc(&c->d_Sfl, E * 9 * c->nf) && dalloc(&c->d_detJ, E * c->n3) && dalloc(&c->d_jinv, E * 9 * c->n3) &&
-            dalloc(&c->d_xsol, E * 3 * c->n3) && dalloc(&c->d_Qf, E * 54 * c->n2) && dalloc(&c->d_Vf, E * 42 * c->n2);
+            dalloc(&c->d_xsol, E * 3 * c->n3) && dalloc(&c->d_Qf[0], E * 54 * c->n2) && dalloc(&c->d_Qf[1], E * 54 * c->n2) &&
+            dalloc(&c->d_Vf, E * 42 * c->n2);
   for (int k = 0; k < 5 && ok; ++k) ok = dalloc(&c->d_U[k], E * 9 * c->n3);
   ok = ok && cudaMalloc(&c->d_ws, sizeof(unsigned long long)) == cudaSuccess;
   if (!ok) return bail(CHORUS_ENOMEM);
@@ -316,7 +379,7 @@ void chorus_free(chorus_ctx* c) {
   cudaFree(c->d_Gm); cudaFree(c->d_Dff); cudaFree(c->d_Efs); cudaFree(c->d_Dfs);
   cudaFree(c->d_Sfl); cudaFree(c->d_detJ); cudaFree(c->d_jinv); cudaFree(c->d_xsol); cudaFree(c->d_krfl);
   for (int k = 0; k < 5; ++k) cudaFree(c->d_U[k]);
-  cudaFree(c->d_Qf); cudaFree(c->d_Vf); cudaFree(c->d_ws);
+  cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_ws);
   for (auto& v : c->prof_ev)
     for (auto& ev : v) {
       cudaEventDestroy(ev.first);
@@ -354,6 +417,7 @@ int chorus_set_state(chorus_ctx* c, const double* q, int on_device) {
   if (!on_device) CU(c, cudaStreamSynchronize(c->stream));
   c->cur = 0;
   c->have_state = true;
+  c->traces_valid = false;
   return CHORUS_OK;
 }
 
@@ -379,7 +443,8 @@ int chorus_residual(chorus_ctx* c, double* r, int on_device) {
   StageOut o{};
   o.Rout = on_device ? r : c->d_U[(c->cur + 1) % 5];
   const double* Qin = c->d_U[c->cur];
-  int rc = DISPATCH_N(c, H::stage(c, Qin, o));
+  double* scratch = c->d_U[(c->cur + 2) % 5];
+  int rc = DISPATCH_N(c, H::stage(c, Qin, o, scratch));
   if (rc) return rc;
   if (!on_device) {
     CU(c, cudaMemcpyAsync(r, o.Rout, sizeof(double) * count, cudaMemcpyDeviceToHost, c->stream));
@@ -400,7 +465,7 @@ int chorus_step(chorus_ctx* c, double dt, int nstages) {
     o.A0 = A0; o.A1 = A1; o.A2 = A2;
     o.c0 = c0; o.c1 = c1; o.c2 = c2; o.bdt = bdt;
     const double* Qin = U[in];
-    return DISPATCH_N(c, H::stage(c, Qin, o));
+    return DISPATCH_N(c, H::stage(c, Qin, o, nullptr));
   };
   int rc = 0;
   if (nstages == 1) {
@@ -481,7 +546,9 @@ int chorus_get_gradient(chorus_ctx* c, double* g, int on_device) {
     return fail(c, CHORUS_ENOMEM, "gradient scratch");
   }
   const double* Qin = c->d_U[c->cur];
-  int rc = DISPATCH_N(c, H::trace(c, Qin));
+  c->traces_valid = false;   // d_Qf[0] is used as scratch below
+  c->qf_cur = 0;
+  int rc = DISPATCH_N(c, H::trace(c, Qin, c->d_Qf[0]));
   if (!rc) rc = DISPATCH_N(c, H::grad(c, Qin, nullptr, tmp));
   if (!rc) {
     double* dst = on_device ? g : tmp2;

@@ -113,6 +113,13 @@ int64_t chorus_launch_count(const chorus_ctx* ctx);
 int chorus_profile(chorus_ctx* ctx, int enable);
 int chorus_profile_read(chorus_ctx* ctx, double* ms /*[3]*/, int64_t* launches /*[3]*/);
 
+/* Measurement: sustained FP64 issue rate of the current device, the denominator of the "alu" roofline.
+ * mode 0: independent DFMA chains on every warp; 1: DMMA.8x8x4 (mma.sync m8n8k4 f64) chains on every warp; 2: half the
+ * warps of every SM sub-partition run DFMA and half DMMA at the same time (tells whether the two share one pipe).
+ * Runs for at least `seconds` on the default stream, synchronises, *tflops (HOST) = 2 x FMA / time / 1e12 in total;
+ * dfma_tflops / dmma_tflops (HOST, may be NULL) = the share of each instruction kind (equal halves in mode 2). */
+int chorus_fp64_peak(int mode, double seconds, double* tflops, double* dfma_tflops, double* dmma_tflops);
+
 #ifdef __cplusplus
 }
 #endif

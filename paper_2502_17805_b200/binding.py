@@ -19,7 +19,7 @@ CHORUS_OK, CHORUS_EINVAL, CHORUS_ENOMEM, CHORUS_ECUDA, CHORUS_ESTATE = 0, -1, -2
 # every symbol include/chorus.h declares
 SYMBOLS = ("chorus_init", "chorus_free", "chorus_set_physics", "chorus_set_state", "chorus_get_state", "chorus_residual",
            "chorus_step", "chorus_max_wavespeed", "chorus_last_error", "chorus_get_geometry", "chorus_get_gradient",
-           "chorus_get_operators", "chorus_launch_count", "chorus_profile", "chorus_profile_read")
+           "chorus_get_operators", "chorus_launch_count", "chorus_profile", "chorus_profile_read", "chorus_fp64_peak")
 
 
 class ChorusError(RuntimeError):
@@ -108,6 +108,20 @@ def get_operators(order):
     if rc:
         raise ChorusError(rc, "chorus_get_operators")
     return xs, xf, Isf, Dfs
+
+
+def fp64_peak(mode=0, seconds=1.0):
+    """Sustained FP64 rate of the current device in TFLOP/s: (total, DFMA share, DMMA share).  mode 0 DFMA, 1 DMMA, 2 both."""
+    import torch
+    if not torch.cuda.is_available():
+        raise ChorusError(CHORUS_ECUDA, "no CUDA device")
+    t, a, b = C.c_double(), C.c_double(), C.c_double()
+    f = lib().chorus_fp64_peak
+    f.argtypes = [C.c_int, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    rc = f(int(mode), float(seconds), C.byref(t), C.byref(a), C.byref(b))
+    if rc:
+        raise ChorusError(rc, "chorus_fp64_peak")
+    return t.value, a.value, b.value
 
 
 class Chorus:

@@ -16,6 +16,7 @@
 #include "basis.h"
 #include "geometry.cuh"
 #include "kernels_stage.cuh"
+#include "peak.cuh"
 
 using namespace chorus;
 
@@ -35,7 +36,7 @@ struct chorus_ctx {
   // operators for the geometry kernel
   double *d_Gm = nullptr, *d_Dff = nullptr, *d_Efs = nullptr, *d_Dfs = nullptr;
   // geometry
-  double *d_Sfl = nullptr, *d_detJ = nullptr, *d_jinv = nullptr, *d_xsol = nullptr, *d_krfl = nullptr;
+  double *d_Sfl = nullptr, *d_detJ = nullptr, *d_jinv = nullptr, *d_xsol = nullptr, *d_krfl = nullptr, *d_nfc = nullptr;
   // state registers (element-major) and face buffers
   double* d_U[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   int cur = 0;
@@ -84,6 +85,7 @@ PhysD to_device_phys(const chorus_physics& p) {
   PhysD d;
   d.gamma = p.gamma; d.gm1 = p.gamma - 1.0; d.R = p.R_gas; d.Cp = p.Cp; d.GM = p.GM; d.Omega = p.Omega;
   d.nu = p.nu; d.kappa = p.kappa; d.eta = p.eta; d.c_h = p.c_h; d.a_psi = p.a_psi; d.q_bottom = p.q_bottom; d.T_top = p.T_top;
+  d.iR = 1.0 / p.R_gas; d.igamma = 1.0 / p.gamma;
   d.bc_inner = p.bc_mag_inner; d.bc_outer = p.bc_mag_outer; d.flags = p.flags;
   return d;
 }
@@ -165,7 +167,7 @@ struct Hot {
     return CHORUS_OK;
   }
   static Geo geo(const chorus_ctx* c) {
-    return Geo{c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl, c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient};
+    return Geo{c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl, c->d_nfc, c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient};
   }
   // one residual evaluation through the pipeline.  io carries Qe and the outputs; the traces of Qe must be in d_Qf[qf_cur].
   static int stage_pipeline(chorus_ctx* c, StageIO io) {
@@ -250,8 +252,19 @@ struct Hot {
     io.Rout = out.Rout;
     io.Qout = out.Qout;
     io.Part = out.Qout ? out.Qout : scratch;
-    io.A0 = out.A0; io.A1 = out.A1; io.A2 = out.A2;
-    io.c0 = out.c0; io.c1 = out.c1; io.c2 = out.c2; io.bdt = out.bdt;
+    io.bdt = out.bdt;
+    {   // split the combination into the evaluated state itself (already on chip) and at most two other registers
+      const double* A[3] = {out.A0, out.A1, out.A2};
+      const double cc[3] = {out.c0, out.c1, out.c2};
+      int k = 0;
+      for (int i = 0; i < 3; ++i) {
+        if (A[i] == nullptr) continue;
+        if (A[i] == Qin) io.cq += cc[i];
+        else if (k == 0) { io.A0 = A[i]; io.c0 = cc[i]; ++k; }
+        else if (k == 1) { io.A1 = A[i]; io.c1 = cc[i]; ++k; }
+        else return fail(c, CHORUS_EINVAL, "more than two foreign stage registers");
+      }
+    }
     return stage_pipeline(c, io);
   }
 };
@@ -287,6 +300,9 @@ int run_geometry(chorus_ctx* c) {
   geometry_kernel<<<(unsigned)c->E, 256, smem, c->stream>>>(c->n, c->ng, c->E, op, c->d_xyz, c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol,
                                                             c->d_krfl, c->phys.kr_scale, c->phys.kr_c[0], c->phys.kr_c[1],
                                                             c->phys.kr_c[2], c->phys.kr_wscale);
+  ++c->launches;
+  CU(c, cudaGetLastError());
+  face_geometry_kernel<<<grid_1d(c, c->E * 6 * c->n2, 256), 256, 0, c->stream>>>(c->n, c->E, c->d_Sfl, c->d_nfc);
   ++c->launches;
   CU(c, cudaGetLastError());
   return CHORUS_OK;
@@ -360,7 +376,7 @@ int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chor
   const size_t E = (size_t)c->E;
   auto dalloc = [&](double** p, size_t count) { return cudaMalloc(p, sizeof(double) * count) == cudaSuccess; };
   bool ok = dalloc(&c->d_Sfl, E * 9 * c->nf) && dalloc(&c->d_detJ, E * c->n3) && dalloc(&c->d_jinv, E * 9 * c->n3) &&
-            dalloc(&c->d_xsol, E * 3 * c->n3) && dalloc(&c->d_Qf[0], E * 54 * c->n2) && dalloc(&c->d_Qf[1], E * 54 * c->n2) &&
+            dalloc(&c->d_xsol, E * 3 * c->n3) && dalloc(&c->d_nfc, E * 24 * c->n2) && dalloc(&c->d_Qf[0], E * 54 * c->n2) && dalloc(&c->d_Qf[1], E * 54 * c->n2) &&
             dalloc(&c->d_Vf, E * 42 * c->n2);
   for (int k = 0; k < 5 && ok; ++k) ok = dalloc(&c->d_U[k], E * 9 * c->n3);
   ok = ok && cudaMalloc(&c->d_ws, sizeof(unsigned long long)) == cudaSuccess;
@@ -377,7 +393,7 @@ void chorus_free(chorus_ctx* c) {
   if (!c) return;
   cudaFree(c->d_xyz); cudaFree(c->d_nbr_elem); cudaFree(c->d_nbr_face); cudaFree(c->d_nbr_orient);
   cudaFree(c->d_Gm); cudaFree(c->d_Dff); cudaFree(c->d_Efs); cudaFree(c->d_Dfs);
-  cudaFree(c->d_Sfl); cudaFree(c->d_detJ); cudaFree(c->d_jinv); cudaFree(c->d_xsol); cudaFree(c->d_krfl);
+  cudaFree(c->d_Sfl); cudaFree(c->d_detJ); cudaFree(c->d_jinv); cudaFree(c->d_xsol); cudaFree(c->d_krfl); cudaFree(c->d_nfc);
   for (int k = 0; k < 5; ++k) cudaFree(c->d_U[k]);
   cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_ws);
   for (auto& v : c->prof_ev)
@@ -588,6 +604,58 @@ int chorus_profile_read(chorus_ctx* c, double* ms, int64_t* launches) {
   }
   return CHORUS_OK;
 }
+
+int chorus_fp64_peak(int mode, double seconds, double* tflops, double* dfma_tflops, double* dmma_tflops) {
+  if (mode < 0 || mode > 2 || !tflops || !(seconds > 0.0)) return CHORUS_EINVAL;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return CHORUS_ECUDA;
+  double* out = nullptr;
+  if (cudaMalloc(&out, sizeof(double)) != cudaSuccess) return CHORUS_ENOMEM;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  const int grid = sms * 8, iters = 4096;
+  auto launch = [&]() {
+    if (mode == 0) fp64_peak_kernel<0><<<grid, 256>>>(iters, 1.0, out);
+    else if (mode == 1) fp64_peak_kernel<1><<<grid, 256>>>(iters, 1.0, out);
+    else fp64_peak_kernel<2><<<grid, 256>>>(iters, 1.0, out);
+  };
+  launch();   // warm-up
+  cudaDeviceSynchronize();
+  // flops of one launch: DFMA warps 64 FMA/thread/iter; DMMA warps 8 x 256 FMA/warp/iter = 64 FMA/thread/iter as well
+  const double flop_per_launch = 2.0 * 64.0 * 256.0 * (double)grid * iters;
+  int reps = 1;
+  float ms = 0.f;
+  for (;;) {
+    cudaEventRecord(e0);
+    for (int r = 0; r < reps; ++r) launch();
+    cudaEventRecord(e1);
+    if (cudaEventSynchronize(e1) != cudaSuccess) break;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (ms * 1e-3 >= seconds || reps > (1 << 20)) break;
+    reps *= 2;
+  }
+  const cudaError_t err = cudaGetLastError();
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  if (err != cudaSuccess || ms <= 0.f) return CHORUS_ECUDA;
+  *tflops = flop_per_launch * reps / (ms * 1e-3) / 1e12;
+  if (dfma_tflops) *dfma_tflops = mode == 0 ? *tflops : mode == 2 ? 0.5 * *tflops : 0.0;
+  if (dmma_tflops) *dmma_tflops = mode == 1 ? *tflops : mode == 2 ? 0.5 * *tflops : 0.0;
+  return CHORUS_OK;
+}
+
+#ifdef CHORUS_PHASE_TIMING
+int chorus_debug_phase_cycles(unsigned long long* out16, int reset) {
+  if (out16 && cudaMemcpyFromSymbol(out16, g_phase_cycles, sizeof(unsigned long long) * 16) != cudaSuccess) return CHORUS_ECUDA;
+  if (reset) {
+    unsigned long long z[16] = {0};
+    if (cudaMemcpyToSymbol(g_phase_cycles, z, sizeof z) != cudaSuccess) return CHORUS_ECUDA;
+  }
+  return CHORUS_OK;
+}
+#endif
 
 int chorus_get_operators(int order, double* xs, double* xf, double* Isf, double* Dfs) {
   if (order < 2 || order > kMaxN) return CHORUS_EINVAL;

@@ -168,4 +168,26 @@ __global__ void geometry_kernel(int n, int ng, int64_t E, GeomOps op, const doub
   }
 }
 
+// Outward unit normal and signed area at the face points, from S^d at the face flux points (O3):
+//   nfc[e][f][0..2][ab] = sigma S/|S|,  nfc[e][f][3][ab] = sigma |S|,  sigma = +1 on the "1" faces, -1 on the "0" faces.
+__global__ void face_geometry_kernel(int n, int64_t E, const double* __restrict__ Sfl, double* __restrict__ nfc) {
+  const int n2 = n * n, nf = n2 * (n + 1);
+  const int64_t total = E * 6 * n2;
+  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+    const int ab = (int)(t % n2), f = (int)((t / n2) % 6);
+    const int64_t e = t / (6 * n2);
+    const int d = f >> 1, m = (f & 1) ? n : 0;
+    const int a = ab % n, b = ab / n;
+    const int fb = d == 0 ? ab * (n + 1) : d == 1 ? b * (n + 1) * n + a : ab;
+    const int ix = fb + m * (d == 0 ? 1 : d == 1 ? n : n2);
+    const double* S = Sfl + (e * 3 + d) * 3 * nf + ix;
+    const double sx = S[0], sy = S[nf], sz = S[2 * nf];
+    const double area = sqrt(sx * sx + sy * sy + sz * sz);
+    const double sg = (f & 1) ? 1.0 : -1.0;
+    const double inv = sg / area;
+    double* o = nfc + (e * 6 + f) * 4 * n2 + ab;
+    o[0] = sx * inv; o[n2] = sy * inv; o[2 * n2] = sz * inv; o[3 * n2] = sg * area;
+  }
+}
+
 }  // namespace chorus

@@ -57,12 +57,11 @@ struct StageIO {
   double* Part;          // diffusion: the main kernel's output (everything but the common viscous face flux), finished by
                          // the face kernel.  Step mode: the new-state buffer itself; residual mode: a scratch buffer.
   double* Rout;          // residual in the INTERFACE layout [9][E][n3], or nullptr (step mode)
-  double* Qout;          // new state (step mode), or nullptr:  Qout = c0*A0 + c1*A1 + c2*A2 + bdt * R
+  double* Qout;          // new state (step mode), or nullptr:  Qout = cq*Qe + c0*A0 + c1*A1 + bdt * R
   double* QfOut;         // face traces of Qout (step mode)
-  const double* A0;      // stage registers; a null pointer contributes nothing
+  const double* A0;      // stage registers other than Qe itself (SSPRK(5,3) needs at most two); nullptr contributes nothing
   const double* A1;
-  const double* A2;
-  double c0, c1, c2, bdt;
+  double cq, c0, c1, bdt;
 };
 
 struct Geo {
@@ -71,6 +70,7 @@ struct Geo {
   const double* jinv;    // [E][3 d][3 p][n3]
   const double* xsol;    // [E][3][n3]
   const double* krfl;    // [E][3 fam][nf] or nullptr
+  const double* nfc;     // [E][6][4][n2]  outward unit normal (3) and sigma |S| at the face points
   const int32_t* nbr_elem;
   const uint8_t* nbr_face;
   const uint8_t* nbr_orient;
@@ -94,6 +94,36 @@ __device__ __forceinline__ void emit_traces(const double* sQ, double* __restrict
     }
     Qf_e[((2 * d) * 9 + v) * I::n2 + ab] = lo;
     Qf_e[((2 * d + 1) * 9 + v) * I::n2 + ab] = hi;
+  }
+}
+
+// Stage the own traces and the neighbours' traces of one element in shared memory (A2, walls :190-198).
+//   sQo[f][v][ab] = own polynomial at the face point;  sQn[f][v][ab] = neighbour's polynomial there, or, on a wall face,
+//   the boundary state Q_b (so that "common solution" = Q_b and "outer state" = Q_b both read sQn).
+template <int N>
+__device__ __forceinline__ void stage_traces_n(int64_t e, const ElemNbr& nb, const PhysD& ph, const double* __restrict__ Qf,
+                                               const double* __restrict__ nfc, double* sQo, double* sQn) {
+  using I = Ix<N>;
+  for (int t = threadIdx.x; t < 6 * I::n2; t += blockDim.x) {
+    const int f = t / I::n2, ab = t % I::n2;
+    double own[9], out[9];
+#pragma unroll
+    for (int v = 0; v < 9; ++v) own[v] = Qf[((e * 6 + f) * 9 + v) * I::n2 + ab];
+    const int ne = nb.ne[f];
+    if (ne >= 0) {
+      const int ab2 = I::orient(nb.no[f], ab);
+      const double* src = Qf + (((int64_t)ne * 6 + nb.nf[f]) * 9) * I::n2 + ab2;
+#pragma unroll
+      for (int v = 0; v < 9; ++v) out[v] = src[v * I::n2];
+    } else {
+      const double* nf_ = nfc + ((e * 6 + f) * 4) * I::n2 + ab;
+      wall_state(ph, ne, own, nf_[0], nf_[I::n2], nf_[2 * I::n2], out);
+    }
+#pragma unroll
+    for (int v = 0; v < 9; ++v) {
+      sQo[(f * 9 + v) * I::n2 + ab] = own[v];
+      sQn[(f * 9 + v) * I::n2 + ab] = out[v];
+    }
   }
 }
 
@@ -126,7 +156,7 @@ __device__ __forceinline__ void vs_fold(VStream& s, const PrimD& p, double Sx, d
 // tauS = tau.S, qS = q.S from the running state
 __device__ __forceinline__ void vs_finish(const PhysD& ph, const VStream& s, const PrimD& p, double Sx, double Sy, double Sz, double kr,
                                           double& t0, double& t1, double& t2, double& qS) {
-  const double ir = 1.0 / p.rho;
+  const double ir = p.ir;
   const double grS = Sx * s.gr0 + Sy * s.gr1 + Sz * s.gr2;
   const double uS = p.u * Sx + p.v * Sy + p.w * Sz;
   const double mu = p.rho * ph.nu;
@@ -138,9 +168,9 @@ __device__ __forceinline__ void vs_finish(const PhysD& ph, const VStream& s, con
   t2 = mi * ((s.mS2 - p.w * grS) + (s.W2 - uS * s.gr2)) + lam * Sz;
   const double u2 = p.u * p.u + p.v * p.v + p.w * p.w;
   const double dpS = ph.gm1 * (s.acc - (p.u * s.mS0 + p.v * s.mS1 + p.w * s.mS2) + 0.5 * u2 * grS);
-  const double Tt = p.p * ir / ph.R;
-  const double dTS = (dpS - p.p * ir * grS) * ir / ph.R;
-  const double dSS = ph.Cp * (dpS / (ph.gamma * p.p) - grS * ir);                  // gradient of Eq. 10
+  const double Tt = p.p * ir * ph.iR;
+  const double dTS = (dpS - p.p * ir * grS) * ir * ph.iR;
+  const double dSS = ph.Cp * (dpS * ph.igamma / p.p - grS * ir);                   // gradient of Eq. 10
   qS = -ph.kappa * p.rho * Tt * dSS - kr * p.rho * ph.Cp * dTS;                    // Eq. 9
 }
 
@@ -182,6 +212,273 @@ __device__ __forceinline__ void vs_flux_wall(const PhysD& ph, int wall, const VS
 #define CHORUS_MAIN_MINBLOCKS 2
 #endif
 
+// first k-step of a product: D = A*B (accumulator starts at zero, no register zeroing)
+__device__ __forceinline__ void dmma884z(double& d0, double& d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%4};\n"
+               : "=d"(d0), "=d"(d1) : "d"(a), "d"(b), "d"(0.0));
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
+// all threads of the CTA: prefetch `bytes` starting at p into L2, one request per 128-byte line
+__device__ __forceinline__ void prefetch_block_l2(const void* p, size_t bytes) {
+  const char* b = (const char*)p;
+  for (size_t o = (size_t)threadIdx.x * 128; o < bytes; o += (size_t)blockDim.x * 128) prefetch_l2(b + o);
+}
+
+// per-thread constants of the DMMA mapping
+template <int N>
+struct LaneK {
+  double bI0, bI1;     // interpolation operand, k-steps 0 and 1
+  double bD0, bD1;     // derivative operand
+  double bG[3];        // BR1 gradient operand
+  int m0, m1;          // flux point of the two columns this thread holds (-1 = padding)
+  int r, c;
+};
+
+// A3 along direction D: d Q_v / d xi_D at the solution points of 8 lines, variables GV0 .. GV0+NGV-1, into sG[(vv*3+D)]
+template <int N, int NGV, int GV0, int D>
+__device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, const double* sQ, const double* sQo, const double* sQn,
+                                         double* sG, int ln, bool lv) {
+  using I = Ix<N>;
+  constexpr int st = D == 0 ? 1 : D == 1 ? N : I::n2;
+  constexpr int KG = (N + 2 + 3) / 4;
+  const int sb = I::sbase(D, ln);
+  const int c = L.c;
+  // operand of k-step s >= 1 in the unified form  a = wX * X[v * sX] + wY * Y[v * sY]
+  const double* X[3];
+  const double* Y[3];
+  int sX[3], sY[3];
+  double wX[3], wY[3];
+#pragma unroll
+  for (int s = 1; s < KG; ++s) {
+    const int k = 4 * s + c;
+    if (k < N) {
+      X[s] = Y[s] = sQ + sb + k * st; sX[s] = sY[s] = I::n3; wX[s] = 1.0; wY[s] = 0.0;
+    } else if (k <= N + 1) {
+      const int f = 2 * D + (k - N);
+      const bool wall = nb.ne[f] < 0;
+      X[s] = sQo + f * 9 * I::n2 + ln; Y[s] = sQn + f * 9 * I::n2 + ln; sX[s] = sY[s] = I::n2;
+      wX[s] = wall ? 0.0 : 0.5; wY[s] = wall ? 1.0 : 0.5;            // BR1 average, or the wall state
+    } else {
+      X[s] = Y[s] = sQ + sb; sX[s] = sY[s] = I::n3; wX[s] = 0.0; wY[s] = 0.0;   // padding: the B operand is zero
+    }
+  }
+  const double* A0 = sQ + sb + c * st;          // k-step 0: k = c < N
+  const bool ok0 = lv && 2 * c < N, ok1 = lv && 2 * c + 1 < N;
+  double* out = sG + D * I::n3 + sb + (2 * c) * st;
+  constexpr int VB = NGV % 3 == 0 ? 3 : 1;      // variables in flight (hides the DMMA latency)
+#pragma unroll
+  for (int v0 = 0; v0 < NGV; v0 += VB) {
+    double d0[VB], d1[VB];
+#pragma unroll
+    for (int j = 0; j < VB; ++j) dmma884z(d0[j], d1[j], A0[(GV0 + v0 + j) * I::n3], L.bG[0]);
+#pragma unroll
+    for (int s = 1; s < KG; ++s)
+#pragma unroll
+      for (int j = 0; j < VB; ++j) {
+        const int v = GV0 + v0 + j;
+        const double a = wX[s] * X[s][v * sX[s]] + wY[s] * Y[s][v * sY[s]];
+        dmma884(d0[j], d1[j], a, L.bG[s]);
+      }
+#pragma unroll
+    for (int j = 0; j < VB; ++j) {
+      if (ok0) out[(v0 + j) * 3 * I::n3] = d0[j];
+      if (ok1) out[(v0 + j) * 3 * I::n3 + st] = d1[j];
+    }
+  }
+}
+
+// A1 + A4 + A5 + A7 along direction D for 8 lines: the register-resident chain
+template <int N, bool DIFF, int D>
+__device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, const ElemNbr& nb, const StageIO& io, const Geo& geo,
+                                          int64_t e, const double* sQ, const double* sG, const double* sFace, const double* sS, double* sR,
+                                          int ln, bool lv) {
+  using I = Ix<N>;
+  constexpr int st = D == 0 ? 1 : D == 1 ? N : I::n2;
+  const int sb = I::sbase(D, ln);
+  const int c = L.c, m0 = L.m0, m1 = L.m1;
+  const int l1 = 4 + c < N ? 4 + c : N - 1;     // second k-step: l = 4 + c, clamped where the B operand is zero anyway
+  const double* A0 = sQ + sb + c * st;
+  const double* A1 = sQ + sb + l1 * st;
+  // A1: Q at the two flux points of this thread
+  double q0[9], q1[9];
+#pragma unroll
+  for (int v = 0; v < 9; ++v) dmma884z(q0[v], q1[v], A0[v * I::n3], L.bI0);
+  if (N > 4) {
+#pragma unroll
+    for (int v = 0; v < 9; ++v) dmma884(q0[v], q1[v], A1[v * I::n3], L.bI1);
+  }
+  // per-slot setup: area vector and the state the fluxes are evaluated on
+  const bool int0 = m0 > 0 && m0 < N, int1 = m1 > 0 && m1 < N;
+  const bool face0 = m0 == 0 || m0 == N, face1 = m1 == 0 || m1 == N;     // m = -1: padding
+  const int fb = I::fbase(D, ln);
+  double S0x = 0.0, S0y = 0.0, S0z = 0.0, S1x = 0.0, S1y = 0.0, S1z = 0.0, kr0 = 0.0, kr1 = 0.0;
+  int fc0 = 0, fc1 = 0;
+  if (int0) {
+    const double* s = sS + (D * 3) * I::nf + fb + m0 * st;
+    S0x = s[0]; S0y = s[I::nf]; S0z = s[2 * I::nf];
+  }
+  if (int1) {
+    const double* s = sS + (D * 3) * I::nf + fb + m1 * st;
+    S1x = s[0]; S1y = s[I::nf]; S1z = s[2 * I::nf];
+  }
+  if (DIFF) {   // face columns: the own-side viscous flux along the outward unit normal, on Q_in (interior) or Q_b (wall)
+    if (face0) {
+      fc0 = 2 * D + (m0 == N ? 1 : 0);
+      const double* nf_ = geo.nfc + ((e * 6 + fc0) * 4) * I::n2 + ln;
+      S0x = nf_[0]; S0y = nf_[I::n2]; S0z = nf_[2 * I::n2];
+      if (nb.ne[fc0] < 0) {
+        double qb[9];
+        wall_state(ph, nb.ne[fc0], q0, S0x, S0y, S0z, qb);
+#pragma unroll
+        for (int v = 0; v < 9; ++v) q0[v] = qb[v];
+      }
+    }
+    if (face1) {
+      fc1 = 2 * D + (m1 == N ? 1 : 0);
+      const double* nf_ = geo.nfc + ((e * 6 + fc1) * 4) * I::n2 + ln;
+      S1x = nf_[0]; S1y = nf_[I::n2]; S1z = nf_[2 * I::n2];
+      if (nb.ne[fc1] < 0) {
+        double qb[9];
+        wall_state(ph, nb.ne[fc1], q1, S1x, S1y, S1z, qb);
+#pragma unroll
+        for (int v = 0; v < 9; ++v) q1[v] = qb[v];
+      }
+    }
+    if (geo.krfl) {
+      if (m0 >= 0) kr0 = geo.krfl[(e * 3 + D) * I::nf + fb + m0 * st];
+      if (m1 >= 0) kr1 = geo.krfl[(e * 3 + D) * I::nf + fb + m1 * st];
+    }
+  }
+  PrimD p0, p1;
+  if (DIFF || int0) p0 = primitives(ph, q0);
+  if (DIFF || int1) p1 = primitives(ph, q1);
+  double Fv0[7], Fv1[7];
+  if (DIFF) {
+    // A4 + Eq. 7-10: stream the gradients of the nine variables through the tensor core, three components at a time
+    VStream s0, s1;
+    const double* G0 = sG + sb + c * st;
+    const double* G1 = sG + sb + l1 * st;
+#define CHORUS_STREAM_VAR(V)                                             \
+  {                                                                      \
+    double ga0, ga1, gb0, gb1, gc0, gc1;                                   \
+    dmma884z(ga0, ga1, G0[(3 * (V)) * I::n3], L.bI0);                    \
+    dmma884z(gb0, gb1, G0[(3 * (V) + 1) * I::n3], L.bI0);                \
+    dmma884z(gc0, gc1, G0[(3 * (V) + 2) * I::n3], L.bI0);                \
+    if (N > 4) {                                                         \
+      dmma884(ga0, ga1, G1[(3 * (V)) * I::n3], L.bI1);                   \
+      dmma884(gb0, gb1, G1[(3 * (V) + 1) * I::n3], L.bI1);               \
+      dmma884(gc0, gc1, G1[(3 * (V) + 2) * I::n3], L.bI1);               \
+    }                                                                    \
+    vs_fold<V>(s0, p0, S0x, S0y, S0z, ga0, gb0, gc0);                    \
+    vs_fold<V>(s1, p1, S1x, S1y, S1z, ga1, gb1, gc1);                    \
+  }
+    CHORUS_STREAM_VAR(0) CHORUS_STREAM_VAR(1) CHORUS_STREAM_VAR(2) CHORUS_STREAM_VAR(3) CHORUS_STREAM_VAR(4)
+    CHORUS_STREAM_VAR(5) CHORUS_STREAM_VAR(6) CHORUS_STREAM_VAR(7) CHORUS_STREAM_VAR(8)
+#undef CHORUS_STREAM_VAR
+    if (face0 && nb.ne[fc0] < 0) vs_flux_wall(ph, nb.ne[fc0], s0, p0, S0x, S0y, S0z, kr0, Fv0);
+    else vs_flux(ph, s0, p0, S0x, S0y, S0z, kr0, Fv0);
+    if (face1 && nb.ne[fc1] < 0) vs_flux_wall(ph, nb.ne[fc1], s1, p1, S1x, S1y, S1z, kr1, Fv1);
+    else vs_flux(ph, s1, p1, S1x, S1y, S1z, kr1, Fv1);
+    if (lv && face0) {
+      double* o = io.Vf + ((e * 6 + fc0) * 7) * I::n2 + ln;
+#pragma unroll
+      for (int k = 0; k < 7; ++k) o[k * I::n2] = Fv0[k];
+    }
+    if (lv && face1) {
+      double* o = io.Vf + ((e * 6 + fc1) * 7) * I::n2 + ln;
+#pragma unroll
+      for (int k = 0; k < 7; ++k) o[k * I::n2] = Fv1[k];
+    }
+  }
+  // A5: F~ at the interior flux points; face columns take the common flux of the face pass; results overwrite q0 / q1
+  if (int0) {
+    double F[9];
+    flux_inviscid<false>(ph, p0, S0x, S0y, S0z, F);
+    q0[0] = F[0]; q0[8] = F[8];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) q0[1 + k] = DIFF ? F[1 + k] - Fv0[k] : F[1 + k];
+  } else if (m0 >= 0) {
+    const double* f = sFace + ((2 * D + (m0 == N ? 1 : 0)) * 9) * I::n2 + ln;
+#pragma unroll
+    for (int v = 0; v < 9; ++v) q0[v] = f[v * I::n2];
+  } else {
+#pragma unroll
+    for (int v = 0; v < 9; ++v) q0[v] = 0.0;
+  }
+  if (int1) {
+    double F[9];
+    flux_inviscid<false>(ph, p1, S1x, S1y, S1z, F);
+    q1[0] = F[0]; q1[8] = F[8];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) q1[1 + k] = DIFF ? F[1 + k] - Fv1[k] : F[1 + k];
+  } else if (m1 >= 0) {
+    const double* f = sFace + ((2 * D + (m1 == N ? 1 : 0)) * 9) * I::n2 + ln;
+#pragma unroll
+    for (int v = 0; v < 9; ++v) q1[v] = f[v * I::n2];
+  } else {
+#pragma unroll
+    for (int v = 0; v < 9; ++v) q1[v] = 0.0;
+  }
+  // A7: derivative of the flux polynomial at the solution points of the line: C fragments reused as A fragments
+  const bool ok0 = lv && 2 * c < N, ok1 = lv && 2 * c + 1 < N;
+  double* out = sR + sb + (2 * c) * st;
+  double r0[9], r1[9];
+#pragma unroll
+  for (int v = 0; v < 9; ++v) dmma884z(r0[v], r1[v], q0[v], L.bD0);
+#pragma unroll
+  for (int v = 0; v < 9; ++v) dmma884(r0[v], r1[v], q1[v], L.bD1);
+#pragma unroll
+  for (int v = 0; v < 9; ++v) {
+    if (ok0) out[v * I::n3] = (D == 0) ? r0[v] : out[v * I::n3] + r0[v];
+    if (ok1) out[v * I::n3 + st] = (D == 0) ? r1[v] : out[v * I::n3 + st] + r1[v];
+  }
+}
+
+// the next element of this CTA: pull what it will read towards L2 while this one computes (part = 0, 1, 2: spread over the phases)
+template <int N, int GRADV>
+__device__ __forceinline__ void prefetch_next(const StageIO& io, const Geo& geo, int64_t en, int part) {
+  using I = Ix<N>;
+  if (part == 0) {
+    prefetch_block_l2(io.Qe + en * 9 * I::n3, sizeof(double) * 9 * I::n3);
+    prefetch_block_l2(io.Qf + en * 54 * I::n2, sizeof(double) * 54 * I::n2);
+    if (GRADV != 0) prefetch_block_l2(geo.jinv + en * 9 * I::n3, sizeof(double) * 9 * I::n3);
+  } else if (part == 1) {
+    prefetch_block_l2(geo.Sfl + en * 9 * I::nf, sizeof(double) * 9 * I::nf);
+    prefetch_block_l2(geo.nfc + en * 24 * I::n2, sizeof(double) * 24 * I::n2);
+    prefetch_block_l2(geo.detJ + en * I::n3, sizeof(double) * I::n3);
+    prefetch_block_l2(geo.xsol + en * 3 * I::n3, sizeof(double) * 3 * I::n3);
+    for (int f = 0; f < 6; ++f) {
+      const int ne = geo.nbr_elem[en * 6 + f];
+      if (ne >= 0) prefetch_block_l2(io.Qf + ((int64_t)ne * 6 + geo.nbr_face[en * 6 + f]) * 9 * I::n2, sizeof(double) * 9 * I::n2);
+    }
+  } else {
+    if (io.A0) prefetch_block_l2(io.A0 + en * 9 * I::n3, sizeof(double) * 9 * I::n3);
+    if (io.A1) prefetch_block_l2(io.A1 + en * 9 * I::n3, sizeof(double) * 9 * I::n3);
+  }
+}
+
+#ifdef CHORUS_PHASE_TIMING   // development aid: per-phase clock cycles of thread 0 of every CTA, summed into g_phase_cycles
+__device__ unsigned long long g_phase_cycles[16];
+#define CHORUS_TICK(k)                                                              \
+  do {                                                                              \
+    if (threadIdx.x == 0) {                                                         \
+      const long long t_ = clock64();                                               \
+      atomicAdd(&g_phase_cycles[k], (unsigned long long)(t_ - tick_));              \
+      tick_ = t_;                                                                   \
+    }                                                                               \
+  } while (0)
+#else
+#define CHORUS_TICK(k) do { } while (0)
+#endif
+
 // GRADV: 0 no gradient needed, 1 gradient of B only (Powell sources without diffusion), 2 all nine variables.
 template <int N, bool DIFF, int GRADV>
 __global__ void __launch_bounds__(Mma<N>::kThreads, CHORUS_MAIN_MINBLOCKS)
@@ -191,322 +488,284 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   static_assert(!DIFF || GRADV == 2, "diffusion needs the gradient of all variables");
   constexpr int NGV = GRADV == 2 ? 9 : GRADV == 1 ? 3 : 0;
   constexpr int GV0 = GRADV == 1 ? 5 : 0;
-  extern __shared__ double sm[];
+  extern __shared__ __align__(16) double sm[];
   double* sQ = sm;                       // [9][n3]
   constexpr int kOwn = 54 * I::n2 > 9 * I::n3 ? 54 * I::n2 : 9 * I::n3;
-  double* sQo = sQ + 9 * I::n3;          // [6][9][n2] own traces; the region is reused as sR [9][n3] after the face pass
-  double* sQn = sQo + kOwn;              // [6][9][n2] neighbour traces / wall states; overwritten by the face fluxes
-  double* sG = sQn + 54 * I::n2;         // [3*NGV][n3]
+  constexpr auto ev = [](int x) { return (x + 1) & ~1; };   // keep every array 16-byte aligned
+  double* sQo = sQ + ev(9 * I::n3);      // [6][9][n2] own traces; reused as sR [9][n3] after the face pass
+  double* sQn = sQo + ev(kOwn);          // [6][9][n2] neighbour traces / wall states; overwritten by the face fluxes
+  double* sS = sQn + ev(54 * I::n2);     // [3 fam][3 comp][nf] S^d at the flux points (cp.async; 9*nf is even)
+  double* sG = sS + 9 * I::nf;           // [3*NGV][n3]
   double* sR = sQo;
   __shared__ ElemNbr nb;
   const OpsC& op = c_ops[N];
-  const int lane = threadIdx.x & 31, r = lane >> 2, c = lane & 3, warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
   // ---- per-lane operator fragments (B operands), fixed for the whole kernel
-  // interpolation: B[k = l][n = col r] = h_l(X_f,m(r));  k-step s covers l = 4s + c
-  const int mB = M::col_m(r);
-  double bI0 = 0.0, bI1 = 0.0;
-  if (mB >= 0) {
-    bI0 = op.Isf[mB * N + c];
-    if (4 + c < N) bI1 = op.Isf[mB * N + 4 + c];
-  }
-  // derivative: B[k = col][n = l_out r] = l'_{m(col)}(X_s,l_out);  k-step s covers col = 2c + s  (the C -> A reuse)
-  const int m0 = M::col_m(2 * c), m1 = M::col_m(2 * c + 1);
-  double bD0 = 0.0, bD1 = 0.0;
-  if (r < N) {
-    if (m0 >= 0) bD0 = op.Dfs[r * (N + 1) + m0];
-    if (m1 >= 0) bD1 = op.Dfs[r * (N + 1) + m1];
-  }
-  // BR1 gradient: x = (q_0..q_{N-1}, common value at m = 0, at m = N), K = N + 2 -> up to 3 k-steps of 4
-  // B[k][n = l_out r]: k < N: Dss[l_out][k]; k = N: Dfs[l_out][0]; k = N+1: Dfs[l_out][N]
-  double bG[3] = {0.0, 0.0, 0.0};
-  if (r < N) {
+  LaneK<N> L;
+  L.r = lane >> 2; L.c = lane & 3;
+  {
+    const int r = L.r, c = L.c;
+    // interpolation: B[k = l][n = col r] = h_l(X_f,m(r));  k-step s covers l = 4s + c
+    const int mB = M::col_m(r);
+    L.bI0 = 0.0; L.bI1 = 0.0;
+    if (mB >= 0) {
+      L.bI0 = op.Isf[mB * N + c];
+      if (4 + c < N) L.bI1 = op.Isf[mB * N + 4 + c];
+    }
+    // derivative: B[k = col][n = l_out r] = l'_{m(col)}(X_s,l_out);  k-step s covers col = 2c + s  (the C -> A reuse)
+    L.m0 = M::col_m(2 * c); L.m1 = M::col_m(2 * c + 1);
+    L.bD0 = 0.0; L.bD1 = 0.0;
+    if (r < N) {
+      if (L.m0 >= 0) L.bD0 = op.Dfs[r * (N + 1) + L.m0];
+      if (L.m1 >= 0) L.bD1 = op.Dfs[r * (N + 1) + L.m1];
+    }
+    // BR1 gradient: x = (q_0..q_{N-1}, common value at m = 0, at m = N), K = N + 2 -> up to 3 k-steps of 4
+    // B[k][n = l_out r]: k < N: Dss[l_out][k]; k = N: Dfs[l_out][0]; k = N+1: Dfs[l_out][N]
 #pragma unroll
     for (int s = 0; s < 3; ++s) {
       const int k = 4 * s + c;
-      if (k < N) bG[s] = op.Dss[r * N + k];
-      else if (k == N) bG[s] = op.Dfs[r * (N + 1)];
-      else if (k == N + 1) bG[s] = op.Dfs[r * (N + 1) + N];
+      L.bG[s] = 0.0;
+      if (r < N) {
+        if (k < N) L.bG[s] = op.Dss[r * N + k];
+        else if (k == N) L.bG[s] = op.Dfs[r * (N + 1)];
+        else if (k == N + 1) L.bG[s] = op.Dfs[r * (N + 1) + N];
+      }
     }
   }
-  constexpr int KG = (N + 2 + 3) / 4;    // k-steps of the gradient product
+  const int line = warp * 8 + L.r;
+  const bool lv = line < I::n2;
+  const int ln = lv ? line : 0;
+
+#ifdef CHORUS_PHASE_TIMING
+  long long tick_ = clock64();
+#endif
+  // connectivity of the element this CTA handles next, fetched one element ahead by threads 0..5
+  int pn_e = 0, pn_f = 0, pn_o = 0;
+  if (threadIdx.x < 6 && (int64_t)blockIdx.x < E) {
+    pn_e = geo.nbr_elem[(int64_t)blockIdx.x * 6 + threadIdx.x];
+    pn_f = geo.nbr_face[(int64_t)blockIdx.x * 6 + threadIdx.x];
+    pn_o = geo.nbr_orient[(int64_t)blockIdx.x * 6 + threadIdx.x];
+  }
+  constexpr bool kVec = (9 * I::n3) % 2 == 0 && (54 * I::n2) % 2 == 0;     // 16-byte cp.async possible for the state and the traces
+  constexpr int P2 = (I::n3 + M::kThreads - 1) / M::kThreads;              // solution points per thread in the pointwise phases
+  constexpr int F2 = (6 * I::n2 + M::kThreads - 1) / M::kThreads;          // face points per thread
 
   for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
     __syncthreads();
-    load_nbr(nb, e, geo.nbr_elem, geo.nbr_face, geo.nbr_orient);
-    for (int t = threadIdx.x; t < 9 * I::n3; t += blockDim.x) sQ[t] = io.Qe[e * 9 * I::n3 + t];
+    CHORUS_TICK(0);
+    // ---- everything this element reads at its start goes to shared memory asynchronously, in one round trip
+    if (threadIdx.x < 6) { nb.ne[threadIdx.x] = pn_e; nb.nf[threadIdx.x] = pn_f; nb.no[threadIdx.x] = pn_o; }
+    {
+      const double* q = io.Qe + e * 9 * I::n3;
+      const double* t = io.Qf + e * 54 * I::n2;
+      const double* g = geo.Sfl + e * 9 * I::nf;
+      if (kVec) {
+        for (int k = threadIdx.x; k < 9 * I::n3 / 2; k += blockDim.x) cp_async16(sQ + 2 * k, q + 2 * k);
+        for (int k = threadIdx.x; k < 54 * I::n2 / 2; k += blockDim.x) cp_async16(sQo + 2 * k, t + 2 * k);
+      } else {
+        for (int k = threadIdx.x; k < 9 * I::n3; k += blockDim.x) cp_async8(sQ + k, q + k);
+        for (int k = threadIdx.x; k < 54 * I::n2; k += blockDim.x) cp_async8(sQo + k, t + k);
+      }
+      for (int k = threadIdx.x; k < 9 * I::nf / 2; k += blockDim.x) cp_async16(sS + 2 * k, g + 2 * k);
+    }
+    __syncthreads();   // nb visible
+    for (int t = threadIdx.x; t < 6 * I::n2; t += blockDim.x) {     // neighbour traces through the orientation map (A2)
+      const int f = t / I::n2, ab = t % I::n2;
+      const int ne = nb.ne[f];
+      if (ne >= 0) {
+        const double* src = io.Qf + (((int64_t)ne * 6 + nb.nf[f]) * 9) * I::n2 + I::orient(nb.no[f], ab);
+#pragma unroll
+        for (int v = 0; v < 9; ++v) cp_async8(sQn + (f * 9 + v) * I::n2 + ab, src + v * I::n2);
+      }
+    }
+    cp_async_commit();
+    {   // the next element of this CTA: its connectivity into registers, everything else towards L2
+      const int64_t en = e + gridDim.x;
+      if (en < E) {
+        if (threadIdx.x < 6) {
+          pn_e = geo.nbr_elem[en * 6 + threadIdx.x];
+          pn_f = geo.nbr_face[en * 6 + threadIdx.x];
+          pn_o = geo.nbr_orient[en * 6 + threadIdx.x];
+        }
+      }
+    }
+    // chain-rule metrics of this thread's solution points: issued now, consumed after the gradient DMMAs
+    double jv[P2][9];
+    if (GRADV != 0) {
+#pragma unroll
+      for (int q = 0; q < P2; ++q) {
+        const int s = threadIdx.x + q * M::kThreads;
+        const int sc = s < I::n3 ? s : 0;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) jv[q][k] = geo.jinv[e * 9 * I::n3 + k * I::n3 + sc];
+      }
+    }
+    cp_async_wait_all();
     __syncthreads();
-    const double* Sfl_e = geo.Sfl + e * 9 * I::nf;
-    stage_traces<N>(e, nb, ph, io.Qf, Sfl_e, sQo, sQn);
+    CHORUS_TICK(1);
+    for (int t = threadIdx.x; t < 6 * I::n2; t += blockDim.x) {     // wall faces: the boundary state Q_b takes the neighbour's place
+      const int f = t / I::n2, ab = t % I::n2;
+      const int ne = nb.ne[f];
+      if (ne < 0) {
+        double own[9], out[9];
+#pragma unroll
+        for (int v = 0; v < 9; ++v) own[v] = sQo[(f * 9 + v) * I::n2 + ab];
+        const double* nf_ = geo.nfc + ((e * 6 + f) * 4) * I::n2 + ab;
+        wall_state(ph, ne, own, nf_[0], nf_[I::n2], nf_[2 * I::n2], out);
+#pragma unroll
+        for (int v = 0; v < 9; ++v) sQn[(f * 9 + v) * I::n2 + ab] = out[v];
+      }
+    }
     __syncthreads();
+    CHORUS_TICK(2);
 
     // ---- A3: BR1 gradient.  d/dxi_d by DMMA (warp = line group, all directions), then the chain rule per point.
     if constexpr (GRADV != 0) {
-      const int line = warp * 8 + r;
-      const bool lv = line < I::n2;
-      const int ln = lv ? line : 0;
-#pragma unroll 1
-      for (int d = 0; d < 3; ++d) {
-        const int st = I::stride(d), sb = I::sbase(d, ln);
-        const int f0 = 2 * d, f1 = 2 * d + 1;
-        const bool w0 = nb.ne[f0] < 0, w1 = nb.ne[f1] < 0;
-#pragma unroll
-        for (int vv = 0; vv < NGV; ++vv) {
-          const int v = GV0 + vv;
-          double d0 = 0.0, d1 = 0.0;
-#pragma unroll
-          for (int s = 0; s < KG; ++s) {
-            const int k = 4 * s + c;
-            double a = 0.0;
-            if (k < N) a = sQ[v * I::n3 + sb + k * st];
-            else if (k == N) {
-              const double o = sQo[(f0 * 9 + v) * I::n2 + ln], nn = sQn[(f0 * 9 + v) * I::n2 + ln];
-              a = w0 ? nn : 0.5 * (o + nn);
-            } else if (k == N + 1) {
-              const double o = sQo[(f1 * 9 + v) * I::n2 + ln], nn = sQn[(f1 * 9 + v) * I::n2 + ln];
-              a = w1 ? nn : 0.5 * (o + nn);
-            }
-            dmma884(d0, d1, a, bG[s]);
-          }
-          if (lv) {
-            if (2 * c < N) sG[(vv * 3 + d) * I::n3 + sb + (2 * c) * st] = d0;
-            if (2 * c + 1 < N) sG[(vv * 3 + d) * I::n3 + sb + (2 * c + 1) * st] = d1;
-          }
-        }
-      }
+      grad_dir<N, NGV, GV0, 0>(L, nb, sQ, sQo, sQn, sG, ln, lv);
+      grad_dir<N, NGV, GV0, 1>(L, nb, sQ, sQo, sQn, sG, ln, lv);
+      grad_dir<N, NGV, GV0, 2>(L, nb, sQ, sQo, sQn, sG, ln, lv);
       __syncthreads();
-      for (int s = threadIdx.x; s < I::n3; s += blockDim.x) {
-        double j[9];
+      CHORUS_TICK(3);
 #pragma unroll
-        for (int k = 0; k < 9; ++k) j[k] = geo.jinv[e * 9 * I::n3 + k * I::n3 + s];
+      for (int q = 0; q < P2; ++q) {
+        const int s = threadIdx.x + q * M::kThreads;
+        if (s < I::n3) {
 #pragma unroll
-        for (int vv = 0; vv < NGV; ++vv) {
-          const double g0 = sG[(vv * 3 + 0) * I::n3 + s], g1 = sG[(vv * 3 + 1) * I::n3 + s], g2 = sG[(vv * 3 + 2) * I::n3 + s];
+          for (int vv = 0; vv < NGV; ++vv) {
+            const double g0 = sG[(vv * 3 + 0) * I::n3 + s], g1 = sG[(vv * 3 + 1) * I::n3 + s], g2 = sG[(vv * 3 + 2) * I::n3 + s];
 #pragma unroll
-          for (int p = 0; p < 3; ++p) sG[(vv * 3 + p) * I::n3 + s] = j[p] * g0 + j[3 + p] * g1 + j[6 + p] * g2;
+            for (int p = 0; p < 3; ++p) sG[(vv * 3 + p) * I::n3 + s] = jv[q][p] * g0 + jv[q][3 + p] * g1 + jv[q][6 + p] * g2;
+          }
         }
       }
     }
+    CHORUS_TICK(4);
 
     // ---- A6: common INVISCID fluxes at the 6 n^2 face points (Rusanov / wall), scaled by sigma |S|, in place over sQn
-    for (int t = threadIdx.x; t < 6 * I::n2; t += blockDim.x) {
-      const int f = t / I::n2, ab = t % I::n2;
-      double nx, ny, nz, area, sg;
-      face_normal<N>(Sfl_e, f, ab, nx, ny, nz, area, sg);
-      double Qo[9], F[9];
+    {
+      double nq[F2][4];
 #pragma unroll
-      for (int v = 0; v < 9; ++v) Qo[v] = sQn[(f * 9 + v) * I::n2 + ab];
-      if (nb.ne[f] >= 0) {
-        double Qi[9];
+      for (int q = 0; q < F2; ++q) {
+        const int t = threadIdx.x + q * M::kThreads;
+        const int tc = t < 6 * I::n2 ? t : 0;
+        const double* nf_ = geo.nfc + (e * 6 + tc / I::n2) * 4 * I::n2 + tc % I::n2;
 #pragma unroll
-        for (int v = 0; v < 9; ++v) Qi[v] = sQo[(f * 9 + v) * I::n2 + ab];
-        flux_rusanov(ph, Qi, Qo, nx, ny, nz, F);
-      } else {
-        const PrimD sb_ = primitives(ph, Qo);          // Qo holds the wall state Q_b
-        flux_inviscid<true>(ph, sb_, nx, ny, nz, F);
+        for (int k = 0; k < 4; ++k) nq[q][k] = nf_[k * I::n2];
       }
-      const double sa = sg * area;
 #pragma unroll
-      for (int v = 0; v < 9; ++v) sQn[(f * 9 + v) * I::n2 + ab] = sa * F[v];
+      for (int q = 0; q < F2; ++q) {
+        const int t = threadIdx.x + q * M::kThreads;
+        if (t < 6 * I::n2) {
+          const int f = t / I::n2, ab = t % I::n2;
+          double Qo[9], F[9];
+#pragma unroll
+          for (int v = 0; v < 9; ++v) Qo[v] = sQn[(f * 9 + v) * I::n2 + ab];
+          if (nb.ne[f] >= 0) {
+            double Qi[9];
+#pragma unroll
+            for (int v = 0; v < 9; ++v) Qi[v] = sQo[(f * 9 + v) * I::n2 + ab];
+            flux_rusanov(ph, Qi, Qo, nq[q][0], nq[q][1], nq[q][2], F);
+          } else {
+            const PrimD sb_ = primitives(ph, Qo);          // Qo holds the wall state Q_b
+            flux_inviscid<true>(ph, sb_, nq[q][0], nq[q][1], nq[q][2], F);
+          }
+#pragma unroll
+          for (int v = 0; v < 9; ++v) sQn[(f * 9 + v) * I::n2 + ab] = nq[q][3] * F[v];
+        }
+      }
     }
-    __syncthreads();   // own traces (sQo) are dead from here on: the region becomes the divergence accumulator sR
+#ifdef CHORUS_L2_PREFETCH
+    if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, 2);
+#endif
+    __syncthreads();              // own traces (sQo) are dead from here on: the region becomes sR
+    CHORUS_TICK(5);
 
     // ---- A1, A4, A5, A7: one DMMA chain per warp and direction
-    {
-      const int line = warp * 8 + r;
-      const bool lv = line < I::n2;
-      const int ln = lv ? line : 0;
-#pragma unroll 1
-      for (int d = 0; d < 3; ++d) {
-        const int st = I::stride(d), sb = I::sbase(d, ln);
-        // A1: Q at the two flux points of this thread
-        double q0[9], q1[9];
+    chain_dir<N, DIFF, 0>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, ln, lv);
+#ifdef CHORUS_L2_PREFETCH
+    if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, 0);
+#endif
+    __syncthreads();
+    CHORUS_TICK(6);
+    chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, ln, lv);
+#ifdef CHORUS_L2_PREFETCH
+    if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, 1);
+#endif
+    __syncthreads();
+    CHORUS_TICK(7);
+    // epilogue inputs of this thread's solution points: issued before the last chain, consumed after it
+    double ej[P2], ex[P2][3];
 #pragma unroll
-        for (int v = 0; v < 9; ++v) {
-          const double a0 = sQ[v * I::n3 + sb + c * st];
-          const double a1 = (4 + c < N) ? sQ[v * I::n3 + sb + (4 + c) * st] : 0.0;
-          q0[v] = 0.0; q1[v] = 0.0;
-          dmma884(q0[v], q1[v], a0, bI0);
-          if (N > 4) dmma884(q0[v], q1[v], a1, bI1);
-        }
-        // per-slot setup: area vector and the state the fluxes are evaluated on
-        const bool int0 = m0 > 0 && m0 < N, int1 = m1 > 0 && m1 < N;
-        const bool face0 = m0 == 0 || m0 == N, face1 = m1 == 0 || m1 == N;     // m = -1: padding
-        double S0x = 0.0, S0y = 0.0, S0z = 0.0, S1x = 0.0, S1y = 0.0, S1z = 0.0, kr0 = 0.0, kr1 = 0.0;
-        int fc0 = 0, fc1 = 0;
-        if (int0) {
-          const int ix = I::fbase(d, ln) + m0 * st;
-          S0x = Sfl_e[(d * 3 + 0) * I::nf + ix]; S0y = Sfl_e[(d * 3 + 1) * I::nf + ix]; S0z = Sfl_e[(d * 3 + 2) * I::nf + ix];
-          if (DIFF && geo.krfl) kr0 = geo.krfl[(e * 3 + d) * I::nf + ix];
-        }
-        if (int1) {
-          const int ix = I::fbase(d, ln) + m1 * st;
-          S1x = Sfl_e[(d * 3 + 0) * I::nf + ix]; S1y = Sfl_e[(d * 3 + 1) * I::nf + ix]; S1z = Sfl_e[(d * 3 + 2) * I::nf + ix];
-          if (DIFF && geo.krfl) kr1 = geo.krfl[(e * 3 + d) * I::nf + ix];
-        }
-        if (DIFF) {   // face columns: the own-side viscous flux along the outward unit normal, on Q_in (interior) or Q_b (wall)
-          if (face0) {
-            fc0 = 2 * d + (m0 == N ? 1 : 0);
-            double area, sg;
-            face_normal<N>(Sfl_e, fc0, ln, S0x, S0y, S0z, area, sg);
-            if (geo.krfl) kr0 = geo.krfl[(e * 3 + d) * I::nf + I::fbase(d, ln) + m0 * st];
-            if (nb.ne[fc0] < 0) {
-              double qb[9];
-              wall_state(ph, nb.ne[fc0], q0, S0x, S0y, S0z, qb);
+    for (int q = 0; q < P2; ++q) {
+      const int s = threadIdx.x + q * M::kThreads;
+      const int sc = s < I::n3 ? s : 0;
+      ej[q] = geo.detJ[e * I::n3 + sc];
 #pragma unroll
-              for (int v = 0; v < 9; ++v) q0[v] = qb[v];
-            }
-          }
-          if (face1) {
-            fc1 = 2 * d + (m1 == N ? 1 : 0);
-            double area, sg;
-            face_normal<N>(Sfl_e, fc1, ln, S1x, S1y, S1z, area, sg);
-            if (geo.krfl) kr1 = geo.krfl[(e * 3 + d) * I::nf + I::fbase(d, ln) + m1 * st];
-            if (nb.ne[fc1] < 0) {
-              double qb[9];
-              wall_state(ph, nb.ne[fc1], q1, S1x, S1y, S1z, qb);
-#pragma unroll
-              for (int v = 0; v < 9; ++v) q1[v] = qb[v];
-            }
-          }
-        }
-        PrimD p0, p1;
-        if (DIFF || int0) p0 = primitives(ph, q0);
-        if (DIFF || int1) p1 = primitives(ph, q1);
-        double Fv0[7], Fv1[7];
-        if (DIFF) {
-          // A4 + Eq. 7-10: stream the gradients of the nine variables through the tensor core, three components at a time
-          VStream s0, s1;
-#define CHORUS_STREAM_VAR(V)                                                                            \
-  {                                                                                                     \
-    double ga0 = 0.0, ga1 = 0.0, gb0 = 0.0, gb1 = 0.0, gc0 = 0.0, gc1 = 0.0;                              \
-    const double* gp = sG + (3 * (V)) * I::n3 + sb + c * st;                                            \
-    dmma884(ga0, ga1, gp[0], bI0);                                                                      \
-    dmma884(gb0, gb1, gp[I::n3], bI0);                                                                  \
-    dmma884(gc0, gc1, gp[2 * I::n3], bI0);                                                              \
-    if (N > 4) {                                                                                        \
-      const bool hi = 4 + c < N;                                                                        \
-      dmma884(ga0, ga1, hi ? gp[4 * st] : 0.0, bI1);                                                    \
-      dmma884(gb0, gb1, hi ? gp[I::n3 + 4 * st] : 0.0, bI1);                                            \
-      dmma884(gc0, gc1, hi ? gp[2 * I::n3 + 4 * st] : 0.0, bI1);                                        \
-    }                                                                                                   \
-    vs_fold<V>(s0, p0, S0x, S0y, S0z, ga0, gb0, gc0);                                                   \
-    vs_fold<V>(s1, p1, S1x, S1y, S1z, ga1, gb1, gc1);                                                   \
-  }
-          CHORUS_STREAM_VAR(0) CHORUS_STREAM_VAR(1) CHORUS_STREAM_VAR(2) CHORUS_STREAM_VAR(3) CHORUS_STREAM_VAR(4)
-          CHORUS_STREAM_VAR(5) CHORUS_STREAM_VAR(6) CHORUS_STREAM_VAR(7) CHORUS_STREAM_VAR(8)
-#undef CHORUS_STREAM_VAR
-          // slot 0
-          if (face0 && nb.ne[fc0] < 0) vs_flux_wall(ph, nb.ne[fc0], s0, p0, S0x, S0y, S0z, kr0, Fv0);
-          else vs_flux(ph, s0, p0, S0x, S0y, S0z, kr0, Fv0);
-          if (face1 && nb.ne[fc1] < 0) vs_flux_wall(ph, nb.ne[fc1], s1, p1, S1x, S1y, S1z, kr1, Fv1);
-          else vs_flux(ph, s1, p1, S1x, S1y, S1z, kr1, Fv1);
-          if (lv) {
-            if (face0) {
-              double* o = io.Vf + ((e * 6 + fc0) * 7) * I::n2 + ln;
-#pragma unroll
-              for (int k = 0; k < 7; ++k) o[k * I::n2] = Fv0[k];
-            }
-            if (face1) {
-              double* o = io.Vf + ((e * 6 + fc1) * 7) * I::n2 + ln;
-#pragma unroll
-              for (int k = 0; k < 7; ++k) o[k * I::n2] = Fv1[k];
-            }
-          }
-        }
-        // A5: F~ at the interior flux points; face columns take the common flux of the face pass; results overwrite q0 / q1
-        if (int0) {
-          double F[9];
-          flux_inviscid<false>(ph, p0, S0x, S0y, S0z, F);
-          q0[0] = F[0]; q0[8] = F[8];
-#pragma unroll
-          for (int k = 0; k < 7; ++k) q0[1 + k] = DIFF ? F[1 + k] - Fv0[k] : F[1 + k];
-        } else if (m0 >= 0) {
-          const int f = 2 * d + (m0 == N ? 1 : 0);
-#pragma unroll
-          for (int v = 0; v < 9; ++v) q0[v] = sQn[(f * 9 + v) * I::n2 + ln];
-        } else {
-#pragma unroll
-          for (int v = 0; v < 9; ++v) q0[v] = 0.0;
-        }
-        if (int1) {
-          double F[9];
-          flux_inviscid<false>(ph, p1, S1x, S1y, S1z, F);
-          q1[0] = F[0]; q1[8] = F[8];
-#pragma unroll
-          for (int k = 0; k < 7; ++k) q1[1 + k] = DIFF ? F[1 + k] - Fv1[k] : F[1 + k];
-        } else if (m1 >= 0) {
-          const int f = 2 * d + (m1 == N ? 1 : 0);
-#pragma unroll
-          for (int v = 0; v < 9; ++v) q1[v] = sQn[(f * 9 + v) * I::n2 + ln];
-        } else {
-#pragma unroll
-          for (int v = 0; v < 9; ++v) q1[v] = 0.0;
-        }
-        // A7: derivative of the flux polynomial at the solution points of the line: C fragments reused as A fragments
-#pragma unroll
-        for (int v = 0; v < 9; ++v) {
-          double r0 = 0.0, r1 = 0.0;
-          dmma884(r0, r1, q0[v], bD0);
-          dmma884(r0, r1, q1[v], bD1);
-          if (lv) {
-            if (2 * c < N) {
-              double* p = sR + v * I::n3 + sb + (2 * c) * st;
-              *p = (d == 0) ? r0 : (*p + r0);
-            }
-            if (2 * c + 1 < N) {
-              double* p = sR + v * I::n3 + sb + (2 * c + 1) * st;
-              *p = (d == 0) ? r1 : (*p + r1);
-            }
-          }
-        }
-        __syncthreads();
-      }
+      for (int k = 0; k < 3; ++k) ex[q][k] = geo.xsol[(e * 3 + k) * I::n3 + sc];
     }
+    chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, ln, lv);
+    __syncthreads();
+    CHORUS_TICK(8);
 
     // ---- A8 + A9
-    for (int s = threadIdx.x; s < I::n3; s += blockDim.x) {
-      double Q[9], R[9];
+    {
+      const bool rk = io.Qout != nullptr;
+      const bool g0 = rk && io.A0 != nullptr, g1 = rk && io.A1 != nullptr;
+      double a0[P2][9], a1[P2][9];     // stage registers read from HBM: all loads in flight before any use
 #pragma unroll
-      for (int v = 0; v < 9; ++v) Q[v] = sQ[v * I::n3 + s];
-      const double rj = -1.0 / geo.detJ[e * I::n3 + s];
-#pragma unroll
-      for (int v = 0; v < 9; ++v) R[v] = sR[v * I::n3 + s] * rj;
-      double divB = 0.0;
-      if (GRADV == 2) divB = sG[15 * I::n3 + s] + sG[19 * I::n3 + s] + sG[23 * I::n3 + s];
-      if (GRADV == 1) divB = sG[0 * I::n3 + s] + sG[4 * I::n3 + s] + sG[8 * I::n3 + s];
-      const PrimD p = primitives(ph, Q);
-      const double* xe = geo.xsol + e * 3 * I::n3;
-      add_sources(ph, p, divB, xe[s], xe[I::n3 + s], xe[2 * I::n3 + s], R);
-      if (io.Qout != nullptr) {        // step mode: Runge-Kutta combination
+      for (int q = 0; q < P2; ++q) {
+        const int s = threadIdx.x + q * M::kThreads;
+        const int sc = s < I::n3 ? s : 0;
 #pragma unroll
         for (int v = 0; v < 9; ++v) {
-          const int64_t ix = (e * 9 + v) * I::n3 + s;
-          double a = io.bdt * R[v];
-          if (io.A0 != nullptr) a += io.c0 * io.A0[ix];
-          if (io.A1 != nullptr) a += io.c1 * io.A1[ix];
-          if (io.A2 != nullptr) a += io.c2 * io.A2[ix];
-          R[v] = a;
+          const int64_t ix = (e * 9 + v) * I::n3 + sc;
+          a0[q][v] = g0 ? io.A0[ix] : 0.0;
+          a1[q][v] = g1 ? io.A1[ix] : 0.0;
         }
       }
-      if (DIFF) {                      // finished by the face kernel
 #pragma unroll
-        for (int v = 0; v < 9; ++v) io.Part[(e * 9 + v) * I::n3 + s] = R[v];
-      } else if (io.Qout != nullptr) {
+      for (int q = 0; q < P2; ++q) {
+        const int s = threadIdx.x + q * M::kThreads;
+        if (s < I::n3) {
+          double Q[9], R[9];
 #pragma unroll
-        for (int v = 0; v < 9; ++v) {
-          io.Qout[(e * 9 + v) * I::n3 + s] = R[v];
-          sQ[v * I::n3 + s] = R[v];     // this thread is the only reader and writer of point s in this phase
+          for (int v = 0; v < 9; ++v) Q[v] = sQ[v * I::n3 + s];
+          const double rj = -1.0 / ej[q];
+#pragma unroll
+          for (int v = 0; v < 9; ++v) R[v] = sR[v * I::n3 + s] * rj;
+          double divB = 0.0;
+          if (GRADV == 2) divB = sG[15 * I::n3 + s] + sG[19 * I::n3 + s] + sG[23 * I::n3 + s];
+          if (GRADV == 1) divB = sG[0 * I::n3 + s] + sG[4 * I::n3 + s] + sG[8 * I::n3 + s];
+          const PrimD p = primitives(ph, Q);
+          add_sources(ph, p, divB, ex[q][0], ex[q][1], ex[q][2], R);
+          if (rk) {                      // step mode: Runge-Kutta combination
+#pragma unroll
+            for (int v = 0; v < 9; ++v) {
+              R[v] = io.bdt * R[v] + io.c0 * a0[q][v] + io.c1 * a1[q][v] + io.cq * Q[v];
+            }
+          }
+          if (DIFF) {                    // finished by the face kernel
+#pragma unroll
+            for (int v = 0; v < 9; ++v) io.Part[(e * 9 + v) * I::n3 + s] = R[v];
+          } else if (rk) {
+#pragma unroll
+            for (int v = 0; v < 9; ++v) {
+              io.Qout[(e * 9 + v) * I::n3 + s] = R[v];
+              sQ[v * I::n3 + s] = R[v];   // this thread is the only reader and writer of point s in this phase
+            }
+          } else {
+#pragma unroll
+            for (int v = 0; v < 9; ++v) io.Rout[((int64_t)v * E + e) * I::n3 + s] = R[v];
+          }
         }
-      } else {
-#pragma unroll
-        for (int v = 0; v < 9; ++v) io.Rout[((int64_t)v * E + e) * I::n3 + s] = R[v];
       }
     }
     if (!DIFF && io.Qout != nullptr) {
       __syncthreads();
       emit_traces<N>(sQ, io.QfOut + e * 54 * I::n2);
     }
+    CHORUS_TICK(9);
   }
 }
 
@@ -515,7 +774,8 @@ constexpr size_t stage_main_smem_bytes() {
   using I = Ix<N>;
   constexpr int NGV = GRADV == 2 ? 9 : GRADV == 1 ? 3 : 0;
   constexpr int kOwn = 54 * I::n2 > 9 * I::n3 ? 54 * I::n2 : 9 * I::n3;
-  return sizeof(double) * (size_t)(9 * I::n3 + kOwn + 54 * I::n2 + 3 * NGV * I::n3);
+  constexpr auto ev = [](int x) { return (x + 1) & ~1; };
+  return sizeof(double) * (size_t)(ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + 9 * I::nf + 3 * NGV * I::n3);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -540,12 +800,9 @@ __global__ void __launch_bounds__(256) stage_face_kernel(int64_t E, StageIO io, 
     load_nbr(nb, e, geo.nbr_elem, geo.nbr_face, geo.nbr_orient);
     for (int t = threadIdx.x; t < 9 * I::n3; t += blockDim.x) sP[t] = io.Part[e * 9 * I::n3 + t];
     __syncthreads();
-    const double* Sfl_e = geo.Sfl + e * 9 * I::nf;
     for (int t = threadIdx.x; t < 6 * I::n2; t += blockDim.x) {
       const int f = t / I::n2, ab = t % I::n2;
-      double nx, ny, nz, area, sg;
-      face_normal<N>(Sfl_e, f, ab, nx, ny, nz, area, sg);
-      const double sa = sg * area;
+      const double sa = geo.nfc[((e * 6 + f) * 4 + 3) * I::n2 + ab];
       const int ne = nb.ne[f];
       const double* mine = io.Vf + ((e * 6 + f) * 7) * I::n2 + ab;
       if (ne >= 0) {

@@ -18,18 +18,21 @@ enum : uint32_t {
 
 struct PhysD {
   double gamma, gm1, R, Cp, GM, Omega, nu, kappa, eta, c_h, a_psi, q_bottom, T_top;
+  double iR, igamma;   // 1/R, 1/gamma
   int bc_inner, bc_outer;
   uint32_t flags;
 };
 
 struct PrimD {
   double rho, u, v, w, p, Bx, By, Bz, psi, E;
+  double ir;   // 1/rho
 };
 
 __device__ __forceinline__ PrimD primitives(const PhysD& ph, const double* Q) {
   PrimD s;
   s.rho = Q[0];
   const double ir = 1.0 / Q[0];
+  s.ir = ir;
   s.u = Q[1] * ir; s.v = Q[2] * ir; s.w = Q[3] * ir;
   s.E = Q[4];
   s.Bx = Q[5]; s.By = Q[6]; s.Bz = Q[7];
@@ -119,7 +122,7 @@ __device__ __forceinline__ void flux_viscous(const PhysD& ph, const PrimD& s, co
 }
 
 __device__ __forceinline__ double fast_speed(const PhysD& ph, const PrimD& s, double nx, double ny, double nz) {
-  const double ir = 1.0 / s.rho;
+  const double ir = s.ir;
   const double a2 = ph.gamma * s.p * ir;
   const double Bn = s.Bx * nx + s.By * ny + s.Bz * nz;
   const double b2 = (s.Bx * s.Bx + s.By * s.By + s.Bz * s.Bz) * ir, bn2 = Bn * Bn * ir;

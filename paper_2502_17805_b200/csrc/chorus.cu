@@ -46,6 +46,7 @@ struct chorus_ctx {
   bool traces_valid = false;              // ... if any does
   double* d_Vf = nullptr;
   unsigned long long* d_ws = nullptr;
+  unsigned* d_arrivals = nullptr;   // per-SM CTA arrival counters of the main kernel
   int64_t launches = 0;
   bool use_mma = true;   // orders 4..7: two-kernel DMMA pipeline (kernels_stage.cuh); CHORUS_KERNELS=scalar selects the
                          // three-kernel shared-memory path that serves the other orders (kernels_residual.cuh)
@@ -128,7 +129,8 @@ struct Hot {
   template <bool DIFF, int GRADV>
   static int main_launch(chorus_ctx* c, const StageIO& io) {
     if constexpr (N >= 4 && N <= 7) {
-      constexpr size_t smem = stage_main_smem_bytes<N, GRADV>();
+      size_t smem = stage_main_smem_bytes<N, GRADV>();
+      if (std::getenv("CHORUS_ONE_CTA")) smem = c->max_smem - 1024;   // experiment: one CTA per SM
       constexpr int threads = Mma<N>::kThreads;
       auto k = stage_main_kernel<N, DIFF, GRADV>;
       CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -253,6 +255,7 @@ struct Hot {
     io.Qout = out.Qout;
     io.Part = out.Qout ? out.Qout : scratch;
     io.bdt = out.bdt;
+    io.sm_arrivals = c->d_arrivals;
     {   // split the combination into the evaluated state itself (already on chip) and at most two other registers
       const double* A[3] = {out.A0, out.A1, out.A2};
       const double cc[3] = {out.c0, out.c1, out.c2};
@@ -380,6 +383,8 @@ int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chor
             dalloc(&c->d_Vf, E * 42 * c->n2);
   for (int k = 0; k < 5 && ok; ++k) ok = dalloc(&c->d_U[k], E * 9 * c->n3);
   ok = ok && cudaMalloc(&c->d_ws, sizeof(unsigned long long)) == cudaSuccess;
+  ok = ok && cudaMalloc(&c->d_arrivals, sizeof(unsigned) * 1024) == cudaSuccess &&
+       cudaMemsetAsync(c->d_arrivals, 0, sizeof(unsigned) * 1024, c->stream) == cudaSuccess;
   if (!ok) return bail(CHORUS_ENOMEM);
   if ((rc = run_geometry(c))) return bail(rc);
   if (cudaStreamSynchronize(c->stream) != cudaSuccess) return bail(CHORUS_ECUDA);   // host mesh buffers may be released by the caller
@@ -395,7 +400,7 @@ void chorus_free(chorus_ctx* c) {
   cudaFree(c->d_Gm); cudaFree(c->d_Dff); cudaFree(c->d_Efs); cudaFree(c->d_Dfs);
   cudaFree(c->d_Sfl); cudaFree(c->d_detJ); cudaFree(c->d_jinv); cudaFree(c->d_xsol); cudaFree(c->d_krfl); cudaFree(c->d_nfc);
   for (int k = 0; k < 5; ++k) cudaFree(c->d_U[k]);
-  cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_ws);
+  cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_ws); cudaFree(c->d_arrivals);
   for (auto& v : c->prof_ev)
     for (auto& ev : v) {
       cudaEventDestroy(ev.first);

@@ -35,9 +35,36 @@ template <int N>
 struct Mma {
   static_assert(N >= 4 && N <= 7, "DMMA chain kernel: orders 4..7");
   using I = Ix<N>;
-  static constexpr int kGroups = (I::n2 + 7) / 8;      // line groups per direction
-  static constexpr int kWarps = kGroups;               // one warp per group
+  // Lines of a direction are handed to warps in groups of 8 (the M dimension of the DMMA).  n^2 = 8 FG + LO: the FG full
+  // groups of a direction are "directional tasks" (compile-time direction); the LO left-over lines of the three directions
+  // are chosen so that no two of them meet in a solution point and are packed together into "tail tasks" whose rows carry
+  // their own direction at run time.  At most 4 warps per CTA: warp w runs on SM sub-partition w % 4, so a fifth warp
+  // would double the load of one FP64 pipe (measured: 5 warps of DMMA take twice as long as 4).
+  static constexpr int FG = I::n2 / 8, LO = I::n2 % 8;
+  static constexpr int kWarps = FG < 4 ? FG : 4;
   static constexpr int kThreads = 32 * kWarps;
+  static constexpr int kTPD = (FG + kWarps - 1) / kWarps;     // directional tasks per warp and direction
+  static constexpr int kTail = (3 * LO + 7) / 8;               // tail tasks per element
+  static_assert(kTail <= kWarps, "tail tasks: one round");
+  // left-over lines (a,b): d = 0: b = 0, a < LO;  d = 1: b = 1, a < LO;  d = 2: a, b >= LO, the first LO of them
+  __host__ __device__ static constexpr bool is_lo(int d, int ab) {
+    const int a = ab % N, b = ab / N;
+    return d == 0 ? (b == 0 && a < LO) : d == 1 ? (b == 1 && a < LO) : (a >= LO && b >= LO && (b - LO) * (N - LO) + (a - LO) < LO);
+  }
+  // slot 0 .. 8 FG - 1: the lines that are not left over, in increasing order; slot 8 FG + i: the i-th left-over line
+  __host__ __device__ static constexpr int line_of(int d, int slot) {
+    int cnt = 0, lo = 0;
+    for (int ab = 0; ab < I::n2; ++ab) {
+      if (is_lo(d, ab)) {
+        if (slot == 8 * FG + lo) return ab;
+        ++lo;
+      } else {
+        if (slot == cnt) return ab;
+        ++cnt;
+      }
+    }
+    return 0;
+  }
   // column j of the 8-wide tile -> flux point index m, or -1 (padding).
   // interior points first; the two face points share the SECOND column of their thread pairs so that one divergent
   // pass serves both (cols 2c+1 of the last two thread columns that hold anything).
@@ -62,6 +89,7 @@ struct StageIO {
   const double* A0;      // stage registers other than Qe itself (SSPRK(5,3) needs at most two); nullptr contributes nothing
   const double* A1;
   double cq, c0, c1, bdt;
+  unsigned* sm_arrivals; // [number of SMs] arrival counters (never reset: only the parity is used)
 };
 
 struct Geo {
@@ -243,13 +271,15 @@ struct LaneK {
 };
 
 // A3 along direction D: d Q_v / d xi_D at the solution points of 8 lines, variables GV0 .. GV0+NGV-1, into sG[(vv*3+D)]
+// D = 3: the direction is the run-time value dd (tail tasks); lv = false: the row is padding (nothing is stored)
 template <int N, int NGV, int GV0, int D>
 __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, const double* sQ, const double* sQo, const double* sQn,
-                                         double* sG, int ln, bool lv) {
+                                         double* sG, int ln, bool lv, int dd = 0) {
   using I = Ix<N>;
-  constexpr int st = D == 0 ? 1 : D == 1 ? N : I::n2;
+  const int d = D < 3 ? D : dd;
+  const int st = D == 0 ? 1 : D == 1 ? N : D == 2 ? I::n2 : I::stride(dd);
   constexpr int KG = (N + 2 + 3) / 4;
-  const int sb = I::sbase(D, ln);
+  const int sb = I::sbase(d, ln);
   const int c = L.c;
   // operand of k-step s >= 1 in the unified form  a = wX * X[v * sX] + wY * Y[v * sY]
   const double* X[3];
@@ -262,7 +292,7 @@ __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, c
     if (k < N) {
       X[s] = Y[s] = sQ + sb + k * st; sX[s] = sY[s] = I::n3; wX[s] = 1.0; wY[s] = 0.0;
     } else if (k <= N + 1) {
-      const int f = 2 * D + (k - N);
+      const int f = 2 * d + (k - N);
       const bool wall = nb.ne[f] < 0;
       X[s] = sQo + f * 9 * I::n2 + ln; Y[s] = sQn + f * 9 * I::n2 + ln; sX[s] = sY[s] = I::n2;
       wX[s] = wall ? 0.0 : 0.5; wY[s] = wall ? 1.0 : 0.5;            // BR1 average, or the wall state
@@ -272,7 +302,7 @@ __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, c
   }
   const double* A0 = sQ + sb + c * st;          // k-step 0: k = c < N
   const bool ok0 = lv && 2 * c < N, ok1 = lv && 2 * c + 1 < N;
-  double* out = sG + D * I::n3 + sb + (2 * c) * st;
+  double* out = sG + d * I::n3 + sb + (2 * c) * st;
   constexpr int VB = NGV % 3 == 0 ? 3 : 1;      // variables in flight (hides the DMMA latency)
 #pragma unroll
   for (int v0 = 0; v0 < NGV; v0 += VB) {
@@ -296,13 +326,15 @@ __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, c
 }
 
 // A1 + A4 + A5 + A7 along direction D for 8 lines: the register-resident chain
+// D = 3: run-time direction dd (tail tasks).  Direction-0 tasks store into sR, all others accumulate.
 template <int N, bool DIFF, int D>
 __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, const ElemNbr& nb, const StageIO& io, const Geo& geo,
                                           int64_t e, const double* sQ, const double* sG, const double* sFace, const double* sS, double* sR,
-                                          int ln, bool lv) {
+                                          int ln, bool lv, int dd = 0) {
   using I = Ix<N>;
-  constexpr int st = D == 0 ? 1 : D == 1 ? N : I::n2;
-  const int sb = I::sbase(D, ln);
+  const int d = D < 3 ? D : dd;
+  const int st = D == 0 ? 1 : D == 1 ? N : D == 2 ? I::n2 : I::stride(dd);
+  const int sb = I::sbase(d, ln);
   const int c = L.c, m0 = L.m0, m1 = L.m1;
   const int l1 = 4 + c < N ? 4 + c : N - 1;     // second k-step: l = 4 + c, clamped where the B operand is zero anyway
   const double* A0 = sQ + sb + c * st;
@@ -318,20 +350,20 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
   // per-slot setup: area vector and the state the fluxes are evaluated on
   const bool int0 = m0 > 0 && m0 < N, int1 = m1 > 0 && m1 < N;
   const bool face0 = m0 == 0 || m0 == N, face1 = m1 == 0 || m1 == N;     // m = -1: padding
-  const int fb = I::fbase(D, ln);
+  const int fb = I::fbase(d, ln);
   double S0x = 0.0, S0y = 0.0, S0z = 0.0, S1x = 0.0, S1y = 0.0, S1z = 0.0, kr0 = 0.0, kr1 = 0.0;
   int fc0 = 0, fc1 = 0;
   if (int0) {
-    const double* s = sS + (D * 3) * I::nf + fb + m0 * st;
+    const double* s = sS + (d * 3) * I::nf + fb + m0 * st;
     S0x = s[0]; S0y = s[I::nf]; S0z = s[2 * I::nf];
   }
   if (int1) {
-    const double* s = sS + (D * 3) * I::nf + fb + m1 * st;
+    const double* s = sS + (d * 3) * I::nf + fb + m1 * st;
     S1x = s[0]; S1y = s[I::nf]; S1z = s[2 * I::nf];
   }
   if (DIFF) {   // face columns: the own-side viscous flux along the outward unit normal, on Q_in (interior) or Q_b (wall)
     if (face0) {
-      fc0 = 2 * D + (m0 == N ? 1 : 0);
+      fc0 = 2 * d + (m0 == N ? 1 : 0);
       const double* nf_ = geo.nfc + ((e * 6 + fc0) * 4) * I::n2 + ln;
       S0x = nf_[0]; S0y = nf_[I::n2]; S0z = nf_[2 * I::n2];
       if (nb.ne[fc0] < 0) {
@@ -342,7 +374,7 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
       }
     }
     if (face1) {
-      fc1 = 2 * D + (m1 == N ? 1 : 0);
+      fc1 = 2 * d + (m1 == N ? 1 : 0);
       const double* nf_ = geo.nfc + ((e * 6 + fc1) * 4) * I::n2 + ln;
       S1x = nf_[0]; S1y = nf_[I::n2]; S1z = nf_[2 * I::n2];
       if (nb.ne[fc1] < 0) {
@@ -353,8 +385,8 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
       }
     }
     if (geo.krfl) {
-      if (m0 >= 0) kr0 = geo.krfl[(e * 3 + D) * I::nf + fb + m0 * st];
-      if (m1 >= 0) kr1 = geo.krfl[(e * 3 + D) * I::nf + fb + m1 * st];
+      if (m0 >= 0) kr0 = geo.krfl[(e * 3 + d) * I::nf + fb + m0 * st];
+      if (m1 >= 0) kr1 = geo.krfl[(e * 3 + d) * I::nf + fb + m1 * st];
     }
   }
   PrimD p0, p1;
@@ -406,7 +438,7 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
 #pragma unroll
     for (int k = 0; k < 7; ++k) q0[1 + k] = DIFF ? F[1 + k] - Fv0[k] : F[1 + k];
   } else if (m0 >= 0) {
-    const double* f = sFace + ((2 * D + (m0 == N ? 1 : 0)) * 9) * I::n2 + ln;
+    const double* f = sFace + ((2 * d + (m0 == N ? 1 : 0)) * 9) * I::n2 + ln;
 #pragma unroll
     for (int v = 0; v < 9; ++v) q0[v] = f[v * I::n2];
   } else {
@@ -420,7 +452,7 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
 #pragma unroll
     for (int k = 0; k < 7; ++k) q1[1 + k] = DIFF ? F[1 + k] - Fv1[k] : F[1 + k];
   } else if (m1 >= 0) {
-    const double* f = sFace + ((2 * D + (m1 == N ? 1 : 0)) * 9) * I::n2 + ln;
+    const double* f = sFace + ((2 * d + (m1 == N ? 1 : 0)) * 9) * I::n2 + ln;
 #pragma unroll
     for (int v = 0; v < 9; ++v) q1[v] = f[v * I::n2];
   } else {
@@ -533,9 +565,29 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       }
     }
   }
-  const int line = warp * 8 + L.r;
-  const bool lv = line < I::n2;
-  const int ln = lv ? line : 0;
+  // lines of this thread's row: directional tasks g = warp, warp + kWarps, ... of each direction, and one row of a tail task
+  int lnd[3][M::kTPD];
+#pragma unroll
+  for (int d = 0; d < 3; ++d)
+#pragma unroll
+    for (int k = 0; k < M::kTPD; ++k) {
+      const int g = warp + k * M::kWarps;
+      lnd[d][k] = M::line_of(d, (g < M::FG ? g : 0) * 8 + L.r);
+    }
+  // tail tasks rotate over the warps (hence over the SM sub-partitions) from element to element, and every second CTA
+  // arriving on an SM starts half a turn ahead (a start-up delay of the second CTA was tried too: no effect, the
+  // two CTAs of an SM drift apart on their own)
+  __shared__ int s_second;
+  if (threadIdx.x == 0) {
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    s_second = (int)(atomicAdd(io.sm_arrivals + smid, 1u) & 1u);
+  }
+  __syncthreads();
+  const bool second = s_second != 0;
+  int tail_rot = second ? M::kWarps / 2 : 0;
+  int tl_d = 0, tl_ln = 0;
+  bool tl_ok = false;
 
 #ifdef CHORUS_PHASE_TIMING
   long long tick_ = clock64();
@@ -554,6 +606,14 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
     __syncthreads();
     CHORUS_TICK(0);
+    const int tw = (warp + tail_rot) % M::kWarps;    // this warp's tail-task index for this element (>= kTail: none)
+    if (M::kTail > 0) {
+      const int q = tw * 8 + L.r;                    // index among the 3 LO left-over lines
+      tl_ok = tw < M::kTail && q < 3 * M::LO;
+      tl_d = tl_ok ? q / (M::LO > 0 ? M::LO : 1) : 0;
+      tl_ln = M::line_of(tl_d, 8 * M::FG + (tl_ok ? q % (M::LO > 0 ? M::LO : 1) : 0));
+      tail_rot = (tail_rot + 1) % M::kWarps;
+    }
     // ---- everything this element reads at its start goes to shared memory asynchronously, in one round trip
     if (threadIdx.x < 6) { nb.ne[threadIdx.x] = pn_e; nb.nf[threadIdx.x] = pn_f; nb.no[threadIdx.x] = pn_o; }
     {
@@ -622,9 +682,14 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
 
     // ---- A3: BR1 gradient.  d/dxi_d by DMMA (warp = line group, all directions), then the chain rule per point.
     if constexpr (GRADV != 0) {
-      grad_dir<N, NGV, GV0, 0>(L, nb, sQ, sQo, sQn, sG, ln, lv);
-      grad_dir<N, NGV, GV0, 1>(L, nb, sQ, sQo, sQn, sG, ln, lv);
-      grad_dir<N, NGV, GV0, 2>(L, nb, sQ, sQo, sQn, sG, ln, lv);
+#pragma unroll
+      for (int k = 0; k < M::kTPD; ++k)
+        if (warp + k * M::kWarps < M::FG) {
+          grad_dir<N, NGV, GV0, 0>(L, nb, sQ, sQo, sQn, sG, lnd[0][k], true);
+          grad_dir<N, NGV, GV0, 1>(L, nb, sQ, sQo, sQn, sG, lnd[1][k], true);
+          grad_dir<N, NGV, GV0, 2>(L, nb, sQ, sQo, sQn, sG, lnd[2][k], true);
+        }
+      if (M::kTail > 0 && tw < M::kTail) grad_dir<N, NGV, GV0, 3>(L, nb, sQ, sQo, sQn, sG, tl_ln, tl_ok, tl_d);
       __syncthreads();
       CHORUS_TICK(3);
 #pragma unroll
@@ -681,14 +746,25 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     __syncthreads();              // own traces (sQo) are dead from here on: the region becomes sR
     CHORUS_TICK(5);
 
-    // ---- A1, A4, A5, A7: one DMMA chain per warp and direction
-    chain_dir<N, DIFF, 0>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, ln, lv);
+    // ---- A1, A4, A5, A7: one DMMA chain per warp and direction.  Direction 0 stores into sR, the others accumulate, so the
+    //      directions are separated by barriers; the points of the left-over direction-0 lines start from zero.
+    if (M::LO > 0) {
+      for (int t = threadIdx.x; t < 9 * M::LO * N; t += blockDim.x) {
+        const int l = t % N, i = (t / N) % M::LO, v = t / (N * M::LO);
+        sR[v * I::n3 + I::sbase(0, M::line_of(0, 8 * M::FG + i)) + l] = 0.0;
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < M::kTPD; ++k)
+      if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 0>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[0][k], true);
 #ifdef CHORUS_L2_PREFETCH
     if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, 0);
 #endif
     __syncthreads();
     CHORUS_TICK(6);
-    chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, ln, lv);
+#pragma unroll
+    for (int k = 0; k < M::kTPD; ++k)
+      if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
 #ifdef CHORUS_L2_PREFETCH
     if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, 1);
 #endif
@@ -704,8 +780,14 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
 #pragma unroll
       for (int k = 0; k < 3; ++k) ex[q][k] = geo.xsol[(e * 3 + k) * I::n3 + sc];
     }
-    chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, ln, lv);
+#pragma unroll
+    for (int k = 0; k < M::kTPD; ++k)
+      if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
     __syncthreads();
+    if (M::kTail > 0) {   // left-over lines of the three directions: no two of them share a solution point
+      if (tw < M::kTail) chain_dir<N, DIFF, 3>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, tl_ln, tl_ok, tl_d);
+      __syncthreads();
+    }
     CHORUS_TICK(8);
 
     // ---- A8 + A9

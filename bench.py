@@ -26,11 +26,11 @@ import numpy as np  # noqa: E402
 METRIC = "SD-MHD DOF-updates/s (sol pts x 9 vars x RK stages)"
 UNIT = "DOF-updates/s"
 NSTAGES = 5
-# Algorithmic HBM bytes per solution point per RK stage (restated in DESIGN.md "Rooflines"):
-# whole stage / the residual+RK kernel's share, for full physics and for diffusion off (Powell sources on).
-ALG_BYTES = {True: (660.0, 532.0), False: (548.0, 476.0)}
-ALG_FLOPS = {True: 3550.0, False: 1370.0}
-FP64_PEAK_TFLOPS = 37.2   # 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz (nominal)
+# Algorithmic work per solution point per RK stage at n = 6 (restated in DESIGN.md 7.3), keyed by
+# "diffusion on": HBM bytes (whole stage, element kernel's share) and flop (whole stage, element kernel's share).
+ALG_BYTES = {True: (660.0, 532.0), False: (548.0, 548.0)}
+ALG_FLOPS = {True: (3550.0, 3360.0), False: (1370.0, 1370.0)}
+FP64_PEAK_TFLOPS = 37.2   # 148 SMs x 4 sub-partitions x 16 FMA/clk x 2 x 1.965 GHz (DMMA measured 37.0)
 
 
 def cpu_sample_workload(w):
@@ -112,8 +112,25 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def max_over_ranks(values, dist=None):
+    """Element-wise max of a list of floats over all ranks (timing rule: multi-GPU numbers are the max over ranks).
+    `dist` is an initialised torch.distributed module or None (single process); works on any backend."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([float(v) for v in values], device=dev, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def job_value(units_per_rank_step, steps, world, ms_max):
+    """Whole-job throughput: the units all ranks processed divided by the slowest rank's time."""
+    return world * units_per_rank_step * steps / (ms_max * 1e-3)
+
+
 def ncu_traffic(workload):
-    """dram bytes per launch of the residual kernel from the committed ncu --set full capture, if one exists."""
+    """dram bytes per launch of the element kernel from the committed ncu --set full capture, if one exists."""
     p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
     if os.path.exists(p):
         try:
@@ -225,40 +242,49 @@ def main():
             g.max_wavespeed()
         barrier()
         e2e_ms = 1e3 * (time.perf_counter() - t0)
-    if dist is not None:
-        t = torch.tensor([ms, e2e_ms or 0.0], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, e2e_max = float(t[0]), float(t[1])
-        e2e_ms = e2e_max if e2e_ms is not None else None
+    ms, e2e_max = max_over_ranks([ms, e2e_ms or 0.0], dist)
+    e2e_ms = e2e_max if e2e_ms is not None else None
+    peaks = None
+    if rank == 0:   # sustained FP64 issue rates of this device (DFMA, DMMA), ~0.5 s each: the "alu" roofline's measured companion
+        try:
+            peaks = dict(dfma_tflops=P.fp64_peak(0, 0.5)[0], dmma_tflops=P.fp64_peak(1, 0.5)[0])
+        except Exception as ex:   # measurement only
+            peaks = dict(error=str(ex))
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return
 
     dof_per_step = pts * 9 * NSTAGES
-    value = world * dof_per_step * args.steps / (ms * 1e-3)
-    peak, peak_src = measured_peaks()
-    res_ms, res_cnt = prof["residual"]
-    res_avg_ms = res_ms / max(res_cnt, 1)
+    value = job_value(dof_per_step, args.steps, world, ms)
+    hbm_peak, peak_src = measured_peaks()
+    main_ms, main_cnt = prof["main"]
+    main_avg_ms = main_ms / max(main_cnt, 1)
     stage_bytes, kernel_bytes = ALG_BYTES[diff]
-    achieved = kernel_bytes * pts / (res_avg_ms * 1e-3) / 1e9 if res_cnt else None
+    stage_flops, kernel_flops = ALG_FLOPS[diff]
+    achieved = kernel_flops * pts / (main_avg_ms * 1e-3) / 1e12 if main_cnt else None        # TFLOP/s of the element kernel
     kernel_ms = {k: (v[0] / max(v[1], 1)) for k, v in prof.items()}
     stage_ms = ms / (args.steps * NSTAGES)
+    t_hbm = stage_bytes * pts / (hbm_peak * 1e9) * 1e3
+    t_alu = stage_flops * pts / (FP64_PEAK_TFLOPS * 1e12) * 1e3
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=warmup, ms_per_step=ms / args.steps,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
                 config=dict(workload=args.workload, mesh=f"6x{w.n_z}x{w.n_z}x{w.n_r} cubed-sphere shell", n_elem=g.E, order=n,
                             solution_points=pts, N_rho=w.N_rho, diffusion=w.diffusion, rk="SSPRK(5,3)",
                             parallelism="replicas" if world > 1 else "single GPU", l2="inputs larger than L2 (state %.0f MB)" % (pts * 72 / 1e6)),
                 clocks=clocks.summary(), gpu_launches=launches,
-                roofline=dict(bound="hbm", kernel="residual_kernel", achieved=achieved, peak=peak, unit="GB/s",
-                              frac=(achieved / peak) if achieved else None, traffic=ncu_traffic(args.workload), peak_source=peak_src,
-                              alg_bytes_per_point=kernel_bytes, kernel_ms=kernel_ms,
-                              kernel_share_of_step={k: v[0] / ms for k, v in prof.items()},
-                              stage=dict(alg_bytes_per_point=stage_bytes, ms=stage_ms, achieved_gbs=stage_bytes * pts / (stage_ms * 1e-3) / 1e9,
-                                         frac_hbm=stage_bytes * pts / (stage_ms * 1e-3) / 1e9 / peak,
-                                         alg_flops_per_point=ALG_FLOPS[diff],
-                                         achieved_fp64_tflops=ALG_FLOPS[diff] * pts / (stage_ms * 1e-3) / 1e12,
-                                         frac_fp64_nominal=ALG_FLOPS[diff] * pts / (stage_ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS)),
+                roofline=dict(bound="alu", kernel="stage_main_kernel", achieved=achieved, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
+                              frac=(achieved / FP64_PEAK_TFLOPS) if achieved else None, traffic=ncu_traffic(args.workload),
+                              peak_source="nominal FP64 pipe: 148 SMs x 4 x 16 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7.3)",
+                              measured_fp64=peaks, alg_flops_per_point=kernel_flops, alg_bytes_per_point=kernel_bytes,
+                              kernel_hbm=dict(achieved_gbs=kernel_bytes * pts / (main_avg_ms * 1e-3) / 1e9 if main_cnt else None,
+                                              peak_gbs=hbm_peak, peak_source=peak_src),
+                              kernel_ms=kernel_ms, kernel_share_of_step={k: v[0] / ms for k, v in prof.items()},
+                              stage=dict(ms=stage_ms, alg_bytes_per_point=stage_bytes, alg_flops_per_point=stage_flops,
+                                         t_hbm_ms=t_hbm, t_alu_ms=t_alu, binding="alu" if t_alu >= t_hbm else "hbm",
+                                         frac_of_binding=max(t_hbm, t_alu) / stage_ms,
+                                         achieved_gbs=stage_bytes * pts / (stage_ms * 1e-3) / 1e9,
+                                         achieved_fp64_tflops=stage_flops * pts / (stage_ms * 1e-3) / 1e12)),
                 wavespeed_after=ws_after)
     if e2e_ms is not None:
         line["e2e"] = dict(value=world * dof_per_step * e2e_steps / (e2e_ms * 1e-3), unit=UNIT, h2d_bytes_per_step=pts * 72,

@@ -109,7 +109,8 @@ int chorus_get_operators(int order, double* xs, double* xf, double* Isf, double*
 int64_t chorus_launch_count(const chorus_ctx* ctx);
 /* Measurement: with profiling enabled every hot-path launch is bracketed by CUDA events on the context's stream.
  * chorus_profile_read synchronises, returns the accumulated device time (ms) and launch count per kernel class
- * -- index 0 face-trace kernel, 1 gradient / viscous-trace kernel, 2 residual + RK kernel -- and resets them. */
+ * -- index 0 face-trace kernel, 1 viscous face kernel (scalar path: gradient kernel), 2 element kernel (stage_main_kernel;
+ * scalar path: residual_kernel) -- and resets them. */
 int chorus_profile(chorus_ctx* ctx, int enable);
 int chorus_profile_read(chorus_ctx* ctx, double* ms /*[3]*/, int64_t* launches /*[3]*/);
 

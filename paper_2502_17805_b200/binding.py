@@ -224,7 +224,8 @@ class Chorus:
         self._check(lib().chorus_profile(self._ctx, int(enable)))
 
     def profile_read(self):
-        """{'trace': (ms, launches), 'grad': ..., 'residual': ...} accumulated since the last read."""
+        """{'trace': (ms, launches), 'face': ..., 'main': ...} accumulated since the last read.  'face' is the viscous face kernel
+        (the gradient kernel on the scalar path), 'main' the element kernel (stage_main_kernel / residual_kernel)."""
         ms, cnt = np.zeros(3), np.zeros(3, np.int64)
         self._check(lib().chorus_profile_read(self._ctx, ms.ctypes.data_as(C.c_void_p), cnt.ctypes.data_as(C.c_void_p)))
-        return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(("trace", "grad", "residual"))}
+        return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(("trace", "face", "main"))}

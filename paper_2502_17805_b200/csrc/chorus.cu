@@ -131,7 +131,7 @@ struct Hot {
     if constexpr (N >= 4 && N <= 7) {
       size_t smem = stage_main_smem_bytes<N, GRADV>();
       if (std::getenv("CHORUS_ONE_CTA")) smem = c->max_smem - 1024;   // experiment: one CTA per SM
-      constexpr int threads = Mma<N>::kThreads;
+      constexpr int threads = kMainThreads;
       auto k = stage_main_kernel<N, DIFF, GRADV>;
       CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       CU(c, cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));

@@ -106,10 +106,10 @@ struct Geo {
 
 // Face traces of the element-resident state sQ [9][n3] -> Qf_e [6][9][n2]  (A1 restricted to the faces; Eq. 19, 21)
 template <int N>
-__device__ __forceinline__ void emit_traces(const double* sQ, double* __restrict__ Qf_e) {
+__device__ __forceinline__ void emit_traces(const double* sQ, double* __restrict__ Qf_e, int tid, int nthreads) {
   using I = Ix<N>;
   const OpsC& op = c_ops[N];
-  for (int t = threadIdx.x; t < 3 * 9 * I::n2; t += blockDim.x) {
+  for (int t = tid; t < 3 * 9 * I::n2; t += nthreads) {
     const int ab = t % I::n2, v = (t / I::n2) % 9, d = t / (9 * I::n2);
     const double* q = sQ + v * I::n3 + I::sbase(d, ab);
     const int st = I::stride(d);
@@ -255,15 +255,27 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
 // all threads of the CTA: prefetch `bytes` starting at p into L2, one request per 128-byte line
-__device__ __forceinline__ void prefetch_block_l2(const void* p, size_t bytes) {
+__device__ __forceinline__ void prefetch_block_l2(const void* p, size_t bytes, int tid, int nthreads) {
   const char* b = (const char*)p;
-  for (size_t o = (size_t)threadIdx.x * 128; o < bytes; o += (size_t)blockDim.x * 128) prefetch_l2(b + o);
+  for (size_t o = (size_t)tid * 128; o < bytes; o += (size_t)nthreads * 128) prefetch_l2(b + o);
 }
+
+// named barriers of the element kernel (id 0 is left to __syncthreads)
+enum : int { kBarChain = 1, kBarHelp = 2, kBarIn = 3, kBarGrad = 4, kBarFaces = 5, kBarRes = 6 };
+__device__ __forceinline__ void bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+template <int R>
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(R)); }
+template <int R>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(R)); }
+
+constexpr int kMainThreads = 256;     // warpgroup 0: chain warps (DMMA), warpgroup 1: helper warps (memory, faces, sources, RK)
+constexpr int kChainRegs = 160, kHelpRegs = 96;   // 128 * (160 + 96) = the CTA's 256 * 128 registers: two CTAs per SM
 
 // per-thread constants of the DMMA mapping
 template <int N>
 struct LaneK {
   double bI0, bI1;     // interpolation operand, k-steps 0 and 1
+  double t0[2], t1[2]; // orders 5, 6: h_l(X_f) of l = 4, 5 at this thread's two columns (the short second k-step is done with DFMA)
   double bD0, bD1;     // derivative operand
   double bG[3];        // BR1 gradient operand
   int m0, m1;          // flux point of the two columns this thread holds (-1 = padding)
@@ -327,10 +339,13 @@ __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, c
 
 // A1 + A4 + A5 + A7 along direction D for 8 lines: the register-resident chain
 // D = 3: run-time direction dd (tail tasks).  Direction-0 tasks store into sR, all others accumulate.
-template <int N, bool DIFF, int D>
+// WAITF: this is the element's first chain task of the warp: the common face fluxes (written by the helper warps beside the
+// chain rule and the first interpolations) are awaited here, just before they are needed, and the left-over direction-0
+// points of sR are zeroed.
+template <int N, bool DIFF, int D, bool WAITF = false>
 __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, const ElemNbr& nb, const StageIO& io, const Geo& geo,
                                           int64_t e, const double* sQ, const double* sG, const double* sFace, const double* sS, double* sR,
-                                          int ln, bool lv, int dd = 0) {
+                                          int ln, bool lv, int dd = 0, int ctid = 0) {
   using I = Ix<N>;
   const int d = D < 3 ? D : dd;
   const int st = D == 0 ? 1 : D == 1 ? N : D == 2 ? I::n2 : I::stride(dd);
@@ -343,7 +358,21 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
   double q0[9], q1[9];
 #pragma unroll
   for (int v = 0; v < 9; ++v) dmma884z(q0[v], q1[v], A0[v * I::n3], L.bI0);
-  if (N > 4) {
+  // second k-step (l = 4 .. N-1).  Orders 5 and 6 have only one or two terms left: four DFMA (8 pipe cycles) instead of a
+  // three-quarters-empty DMMA (16 pipe cycles); every thread of a row reads the same two values (broadcast).
+  constexpr bool kScalarTail = false;   // tried for N = 5, 6: fewer pipe cycles, but the extra live registers spill at 160 and the chains get slower
+  const double* T4 = sQ + sb + 4 * st;           // solution value l = 4 of this thread's line (l = 5: + st)
+  if (kScalarTail) {
+#pragma unroll
+    for (int v = 0; v < 9; ++v) {
+      const double x4 = T4[v * I::n3];
+      q0[v] = fma(x4, L.t0[0], q0[v]); q1[v] = fma(x4, L.t1[0], q1[v]);
+      if (N == 6) {
+        const double x5 = T4[v * I::n3 + st];
+        q0[v] = fma(x5, L.t0[1], q0[v]); q1[v] = fma(x5, L.t1[1], q1[v]);
+      }
+    }
+  } else if (N > 4) {
 #pragma unroll
     for (int v = 0; v < 9; ++v) dmma884(q0[v], q1[v], A1[v * I::n3], L.bI1);
   }
@@ -398,13 +427,25 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
     VStream s0, s1;
     const double* G0 = sG + sb + c * st;
     const double* G1 = sG + sb + l1 * st;
+    const double* G4 = sG + sb + 4 * st;
 #define CHORUS_STREAM_VAR(V)                                             \
   {                                                                      \
     double ga0, ga1, gb0, gb1, gc0, gc1;                                   \
     dmma884z(ga0, ga1, G0[(3 * (V)) * I::n3], L.bI0);                    \
     dmma884z(gb0, gb1, G0[(3 * (V) + 1) * I::n3], L.bI0);                \
     dmma884z(gc0, gc1, G0[(3 * (V) + 2) * I::n3], L.bI0);                \
-    if (N > 4) {                                                         \
+    if (kScalarTail) {                                                   \
+      const double xa = G4[(3 * (V)) * I::n3], xb = G4[(3 * (V) + 1) * I::n3], xc = G4[(3 * (V) + 2) * I::n3]; \
+      ga0 = fma(xa, L.t0[0], ga0); ga1 = fma(xa, L.t1[0], ga1);          \
+      gb0 = fma(xb, L.t0[0], gb0); gb1 = fma(xb, L.t1[0], gb1);          \
+      gc0 = fma(xc, L.t0[0], gc0); gc1 = fma(xc, L.t1[0], gc1);          \
+      if (N == 6) {                                                      \
+        const double ya = G4[(3 * (V)) * I::n3 + st], yb = G4[(3 * (V) + 1) * I::n3 + st], yc = G4[(3 * (V) + 2) * I::n3 + st]; \
+        ga0 = fma(ya, L.t0[1], ga0); ga1 = fma(ya, L.t1[1], ga1);        \
+        gb0 = fma(yb, L.t0[1], gb0); gb1 = fma(yb, L.t1[1], gb1);        \
+        gc0 = fma(yc, L.t0[1], gc0); gc1 = fma(yc, L.t1[1], gc1);        \
+      }                                                                  \
+    } else if (N > 4) {                                                  \
       dmma884(ga0, ga1, G1[(3 * (V)) * I::n3], L.bI1);                   \
       dmma884(gb0, gb1, G1[(3 * (V) + 1) * I::n3], L.bI1);               \
       dmma884(gc0, gc1, G1[(3 * (V) + 2) * I::n3], L.bI1);               \
@@ -428,6 +469,18 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
       double* o = io.Vf + ((e * 6 + fc1) * 7) * I::n2 + ln;
 #pragma unroll
       for (int k = 0; k < 7; ++k) o[k * I::n2] = Fv1[k];
+    }
+  }
+  if (WAITF) {
+    bar_sync(kBarFaces, kMainThreads);     // common face fluxes are in sFace; own traces are dead: their region becomes sR
+    // Direction 0 stores into sR, the others accumulate; the points of the left-over direction-0 lines, which no direction-0
+    // task touches, start from zero (they are first accumulated into after the next chain-warp barrier).
+    using MM = Mma<N>;
+    if (MM::LO > 0) {
+      for (int t = ctid; t < 9 * MM::LO * N; t += 32 * MM::kWarps) {
+        const int l = t % N, i = (t / N) % MM::LO, v = t / (N * MM::LO);
+        sR[v * I::n3 + I::sbase(0, MM::line_of(0, 8 * MM::FG + i)) + l] = 0.0;
+      }
     }
   }
   // A5: F~ at the interior flux points; face columns take the common flux of the face pass; results overwrite q0 / q1
@@ -474,30 +527,27 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
   }
 }
 
-// the next element of this CTA: pull what it will read towards L2 while this one computes (part = 0, 1, 2: spread over the phases)
+// the next element of this CTA: pull what it will read towards L2 (issued by the helper warps while the chains run)
 template <int N, int GRADV>
-__device__ __forceinline__ void prefetch_next(const StageIO& io, const Geo& geo, int64_t en, int part) {
+__device__ __forceinline__ void prefetch_next(const StageIO& io, const Geo& geo, int64_t en, int ne, int nf, int tid, int nthreads) {
   using I = Ix<N>;
-  if (part == 0) {
-    prefetch_block_l2(io.Qe + en * 9 * I::n3, sizeof(double) * 9 * I::n3);
-    prefetch_block_l2(io.Qf + en * 54 * I::n2, sizeof(double) * 54 * I::n2);
-    if (GRADV != 0) prefetch_block_l2(geo.jinv + en * 9 * I::n3, sizeof(double) * 9 * I::n3);
-  } else if (part == 1) {
-    prefetch_block_l2(geo.Sfl + en * 9 * I::nf, sizeof(double) * 9 * I::nf);
-    prefetch_block_l2(geo.nfc + en * 24 * I::n2, sizeof(double) * 24 * I::n2);
-    prefetch_block_l2(geo.detJ + en * I::n3, sizeof(double) * I::n3);
-    prefetch_block_l2(geo.xsol + en * 3 * I::n3, sizeof(double) * 3 * I::n3);
-    for (int f = 0; f < 6; ++f) {
-      const int ne = geo.nbr_elem[en * 6 + f];
-      if (ne >= 0) prefetch_block_l2(io.Qf + ((int64_t)ne * 6 + geo.nbr_face[en * 6 + f]) * 9 * I::n2, sizeof(double) * 9 * I::n2);
-    }
-  } else {
-    if (io.A0) prefetch_block_l2(io.A0 + en * 9 * I::n3, sizeof(double) * 9 * I::n3);
-    if (io.A1) prefetch_block_l2(io.A1 + en * 9 * I::n3, sizeof(double) * 9 * I::n3);
+  prefetch_block_l2(io.Qe + en * 9 * I::n3, sizeof(double) * 9 * I::n3, tid, nthreads);
+  prefetch_block_l2(io.Qf + en * 54 * I::n2, sizeof(double) * 54 * I::n2, tid, nthreads);
+  prefetch_block_l2(geo.Sfl + en * 9 * I::nf, sizeof(double) * 9 * I::nf, tid, nthreads);
+  prefetch_block_l2(geo.nfc + en * 24 * I::n2, sizeof(double) * 24 * I::n2, tid, nthreads);
+  prefetch_block_l2(geo.detJ + en * I::n3, sizeof(double) * I::n3, tid, nthreads);
+  prefetch_block_l2(geo.xsol + en * 3 * I::n3, sizeof(double) * 3 * I::n3, tid, nthreads);
+  if (GRADV != 0) prefetch_block_l2(geo.jinv + en * 9 * I::n3, sizeof(double) * 9 * I::n3, tid, nthreads);
+  if (io.A0) prefetch_block_l2(io.A0 + en * 9 * I::n3, sizeof(double) * 9 * I::n3, tid, nthreads);
+  if (io.A1) prefetch_block_l2(io.A1 + en * 9 * I::n3, sizeof(double) * 9 * I::n3, tid, nthreads);
+  // threads 0..5 hold the neighbour (ne, nf) of face tid: one neighbour face block each, 9 n^2 doubles
+  if (tid < 6 && ne >= 0) {
+    const char* b = (const char*)(io.Qf + ((int64_t)ne * 6 + nf) * 9 * I::n2);
+    for (size_t o = 0; o < sizeof(double) * 9 * I::n2; o += 128) prefetch_l2(b + o);
   }
 }
 
-#ifdef CHORUS_PHASE_TIMING   // development aid: per-phase clock cycles of thread 0 of every CTA, summed into g_phase_cycles
+#ifdef CHORUS_PHASE_TIMING   // development aid: per-phase clock cycles of the first chain thread of every CTA, summed into g_phase_cycles
 __device__ unsigned long long g_phase_cycles[16];
 #define CHORUS_TICK(k)                                                              \
   do {                                                                              \
@@ -512,8 +562,17 @@ __device__ unsigned long long g_phase_cycles[16];
 #endif
 
 // GRADV: 0 no gradient needed, 1 gradient of B only (Powell sources without diffusion), 2 all nine variables.
+//
+// One CTA = two warpgroups working on ONE element at a time:
+//   chain warps (threads 0..127, up to 4 active warps = one per SM sub-partition; 160 registers): the DMMA work -- gradient
+//     tasks, chain rule, the A1/A4/A5/A7 chains;
+//   helper warps (threads 128..255; 96 registers): everything that waits on memory or is pointwise -- cp.async of the element's
+//     inputs, wall states, the Rusanov face pass (beside the gradient), and, beside the chains, the sources and the
+//     Runge-Kutta register loads, so that after the chains only  out = w * sR + K  is left.
+// Barriers per element: IN (inputs ready) -> GRAD (gradient DMMAs done, face fluxes in registers) -> CHAINRULE (gradient and
+// face fluxes in shared memory) -> RES (divergence accumulated).
 template <int N, bool DIFF, int GRADV>
-__global__ void __launch_bounds__(Mma<N>::kThreads, CHORUS_MAIN_MINBLOCKS)
+__global__ void __launch_bounds__(kMainThreads, 2)
 stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   using I = Ix<N>;
   using M = Mma<N>;
@@ -530,53 +589,6 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   double* sG = sS + 9 * I::nf;           // [3*NGV][n3]
   double* sR = sQo;
   __shared__ ElemNbr nb;
-  const OpsC& op = c_ops[N];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-
-  // ---- per-lane operator fragments (B operands), fixed for the whole kernel
-  LaneK<N> L;
-  L.r = lane >> 2; L.c = lane & 3;
-  {
-    const int r = L.r, c = L.c;
-    // interpolation: B[k = l][n = col r] = h_l(X_f,m(r));  k-step s covers l = 4s + c
-    const int mB = M::col_m(r);
-    L.bI0 = 0.0; L.bI1 = 0.0;
-    if (mB >= 0) {
-      L.bI0 = op.Isf[mB * N + c];
-      if (4 + c < N) L.bI1 = op.Isf[mB * N + 4 + c];
-    }
-    // derivative: B[k = col][n = l_out r] = l'_{m(col)}(X_s,l_out);  k-step s covers col = 2c + s  (the C -> A reuse)
-    L.m0 = M::col_m(2 * c); L.m1 = M::col_m(2 * c + 1);
-    L.bD0 = 0.0; L.bD1 = 0.0;
-    if (r < N) {
-      if (L.m0 >= 0) L.bD0 = op.Dfs[r * (N + 1) + L.m0];
-      if (L.m1 >= 0) L.bD1 = op.Dfs[r * (N + 1) + L.m1];
-    }
-    // BR1 gradient: x = (q_0..q_{N-1}, common value at m = 0, at m = N), K = N + 2 -> up to 3 k-steps of 4
-    // B[k][n = l_out r]: k < N: Dss[l_out][k]; k = N: Dfs[l_out][0]; k = N+1: Dfs[l_out][N]
-#pragma unroll
-    for (int s = 0; s < 3; ++s) {
-      const int k = 4 * s + c;
-      L.bG[s] = 0.0;
-      if (r < N) {
-        if (k < N) L.bG[s] = op.Dss[r * N + k];
-        else if (k == N) L.bG[s] = op.Dfs[r * (N + 1)];
-        else if (k == N + 1) L.bG[s] = op.Dfs[r * (N + 1) + N];
-      }
-    }
-  }
-  // lines of this thread's row: directional tasks g = warp, warp + kWarps, ... of each direction, and one row of a tail task
-  int lnd[3][M::kTPD];
-#pragma unroll
-  for (int d = 0; d < 3; ++d)
-#pragma unroll
-    for (int k = 0; k < M::kTPD; ++k) {
-      const int g = warp + k * M::kWarps;
-      lnd[d][k] = M::line_of(d, (g < M::FG ? g : 0) * 8 + L.r);
-    }
-  // tail tasks rotate over the warps (hence over the SM sub-partitions) from element to element, and every second CTA
-  // arriving on an SM starts half a turn ahead (a start-up delay of the second CTA was tried too: no effect, the
-  // two CTAs of an SM drift apart on their own)
   __shared__ int s_second;
   if (threadIdx.x == 0) {
     unsigned smid;
@@ -584,249 +596,321 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     s_second = (int)(atomicAdd(io.sm_arrivals + smid, 1u) & 1u);
   }
   __syncthreads();
-  const bool second = s_second != 0;
-  int tail_rot = second ? M::kWarps / 2 : 0;
-  int tl_d = 0, tl_ln = 0;
-  bool tl_ok = false;
+  const int wg = threadIdx.x >> 7, tid = threadIdx.x & 127;
+  constexpr int H = 128;                 // threads per warpgroup
 
+  if (wg == 0) {
+    // =============================================== chain warps ===============================================
+    setmaxnreg_inc<kChainRegs>();
+    const OpsC& op = c_ops[N];
+    const int lane = tid & 31, warp = tid >> 5;
+    const bool active = warp < M::kWarps;
+    // ---- per-lane operator fragments (B operands), fixed for the whole kernel
+    LaneK<N> L;
+    L.r = lane >> 2; L.c = lane & 3;
+    {
+      const int r = L.r, c = L.c;
+      // interpolation: B[k = l][n = col r] = h_l(X_f,m(r));  k-step s covers l = 4s + c
+      const int mB = M::col_m(r);
+      L.bI0 = 0.0; L.bI1 = 0.0;
+      L.t0[0] = L.t0[1] = L.t1[0] = L.t1[1] = 0.0;
+      if (mB >= 0) {
+        L.bI0 = op.Isf[mB * N + c];
+        if (4 + c < N) L.bI1 = op.Isf[mB * N + 4 + c];
+      }
+      // derivative: B[k = col][n = l_out r] = l'_{m(col)}(X_s,l_out);  k-step s covers col = 2c + s  (the C -> A reuse)
+      L.m0 = M::col_m(2 * c); L.m1 = M::col_m(2 * c + 1);
+#pragma unroll
+      for (int l = 4; l < N && l < 6; ++l) {
+        if (L.m0 >= 0) L.t0[l - 4] = op.Isf[L.m0 * N + l];
+        if (L.m1 >= 0) L.t1[l - 4] = op.Isf[L.m1 * N + l];
+      }
+      L.bD0 = 0.0; L.bD1 = 0.0;
+      if (r < N) {
+        if (L.m0 >= 0) L.bD0 = op.Dfs[r * (N + 1) + L.m0];
+        if (L.m1 >= 0) L.bD1 = op.Dfs[r * (N + 1) + L.m1];
+      }
+      // BR1 gradient: x = (q_0..q_{N-1}, common value at m = 0, at m = N), K = N + 2 -> up to 3 k-steps of 4
+      // B[k][n = l_out r]: k < N: Dss[l_out][k]; k = N: Dfs[l_out][0]; k = N+1: Dfs[l_out][N]
+#pragma unroll
+      for (int s = 0; s < 3; ++s) {
+        const int k = 4 * s + c;
+        L.bG[s] = 0.0;
+        if (r < N) {
+          if (k < N) L.bG[s] = op.Dss[r * N + k];
+          else if (k == N) L.bG[s] = op.Dfs[r * (N + 1)];
+          else if (k == N + 1) L.bG[s] = op.Dfs[r * (N + 1) + N];
+        }
+      }
+    }
+    // lines of this thread's row: directional tasks g = warp, warp + kWarps, ... of each direction, and one row of a tail task
+    int lnd[3][M::kTPD];
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+#pragma unroll
+      for (int k = 0; k < M::kTPD; ++k) {
+        const int g = warp + k * M::kWarps;
+        lnd[d][k] = M::line_of(d, (g < M::FG ? g : 0) * 8 + L.r);
+      }
+    // tail tasks rotate over the warps (hence over the SM sub-partitions) from element to element, and every second CTA
+    // arriving on an SM starts half a turn ahead
+    int tail_rot = s_second ? M::kWarps / 2 : 0;
+    constexpr int P2 = (I::n3 + H - 1) / H;     // solution points per chain thread in the chain rule
 #ifdef CHORUS_PHASE_TIMING
-  long long tick_ = clock64();
+    long long tick_ = clock64();
 #endif
-  // connectivity of the element this CTA handles next, fetched one element ahead by threads 0..5
-  int pn_e = 0, pn_f = 0, pn_o = 0;
-  if (threadIdx.x < 6 && (int64_t)blockIdx.x < E) {
-    pn_e = geo.nbr_elem[(int64_t)blockIdx.x * 6 + threadIdx.x];
-    pn_f = geo.nbr_face[(int64_t)blockIdx.x * 6 + threadIdx.x];
-    pn_o = geo.nbr_orient[(int64_t)blockIdx.x * 6 + threadIdx.x];
-  }
-  constexpr bool kVec = (9 * I::n3) % 2 == 0 && (54 * I::n2) % 2 == 0;     // 16-byte cp.async possible for the state and the traces
-  constexpr int P2 = (I::n3 + M::kThreads - 1) / M::kThreads;              // solution points per thread in the pointwise phases
-  constexpr int F2 = (6 * I::n2 + M::kThreads - 1) / M::kThreads;          // face points per thread
-
-  for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
-    __syncthreads();
-    CHORUS_TICK(0);
-    const int tw = (warp + tail_rot) % M::kWarps;    // this warp's tail-task index for this element (>= kTail: none)
-    if (M::kTail > 0) {
-      const int q = tw * 8 + L.r;                    // index among the 3 LO left-over lines
-      tl_ok = tw < M::kTail && q < 3 * M::LO;
-      tl_d = tl_ok ? q / (M::LO > 0 ? M::LO : 1) : 0;
-      tl_ln = M::line_of(tl_d, 8 * M::FG + (tl_ok ? q % (M::LO > 0 ? M::LO : 1) : 0));
-      tail_rot = (tail_rot + 1) % M::kWarps;
-    }
-    // ---- everything this element reads at its start goes to shared memory asynchronously, in one round trip
-    if (threadIdx.x < 6) { nb.ne[threadIdx.x] = pn_e; nb.nf[threadIdx.x] = pn_f; nb.no[threadIdx.x] = pn_o; }
-    {
-      const double* q = io.Qe + e * 9 * I::n3;
-      const double* t = io.Qf + e * 54 * I::n2;
-      const double* g = geo.Sfl + e * 9 * I::nf;
-      if (kVec) {
-        for (int k = threadIdx.x; k < 9 * I::n3 / 2; k += blockDim.x) cp_async16(sQ + 2 * k, q + 2 * k);
-        for (int k = threadIdx.x; k < 54 * I::n2 / 2; k += blockDim.x) cp_async16(sQo + 2 * k, t + 2 * k);
-      } else {
-        for (int k = threadIdx.x; k < 9 * I::n3; k += blockDim.x) cp_async8(sQ + k, q + k);
-        for (int k = threadIdx.x; k < 54 * I::n2; k += blockDim.x) cp_async8(sQo + k, t + k);
+    for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
+      CHORUS_TICK(0);
+      int tw = M::kWarps, tl_d = 0, tl_ln = 0;
+      bool tl_ok = false;
+      if (M::kTail > 0 && active) {
+        tw = (warp + tail_rot) % M::kWarps;          // this warp's tail-task index for this element (>= kTail: none)
+        const int q = tw * 8 + L.r;                  // index among the 3 LO left-over lines
+        tl_ok = tw < M::kTail && q < 3 * M::LO;
+        tl_d = tl_ok ? q / (M::LO > 0 ? M::LO : 1) : 0;
+        tl_ln = M::line_of(tl_d, 8 * M::FG + (tl_ok ? q % (M::LO > 0 ? M::LO : 1) : 0));
+        tail_rot = (tail_rot + 1) % M::kWarps;
       }
-      for (int k = threadIdx.x; k < 9 * I::nf / 2; k += blockDim.x) cp_async16(sS + 2 * k, g + 2 * k);
-    }
-    __syncthreads();   // nb visible
-    for (int t = threadIdx.x; t < 6 * I::n2; t += blockDim.x) {     // neighbour traces through the orientation map (A2)
-      const int f = t / I::n2, ab = t % I::n2;
-      const int ne = nb.ne[f];
-      if (ne >= 0) {
-        const double* src = io.Qf + (((int64_t)ne * 6 + nb.nf[f]) * 9) * I::n2 + I::orient(nb.no[f], ab);
+      // chain-rule metrics of this thread's solution points: issued now, consumed after the gradient DMMAs
+      double jv[P2][9];
+      if (GRADV != 0) {
 #pragma unroll
-        for (int v = 0; v < 9; ++v) cp_async8(sQn + (f * 9 + v) * I::n2 + ab, src + v * I::n2);
-      }
-    }
-    cp_async_commit();
-    {   // the next element of this CTA: its connectivity into registers, everything else towards L2
-      const int64_t en = e + gridDim.x;
-      if (en < E) {
-        if (threadIdx.x < 6) {
-          pn_e = geo.nbr_elem[en * 6 + threadIdx.x];
-          pn_f = geo.nbr_face[en * 6 + threadIdx.x];
-          pn_o = geo.nbr_orient[en * 6 + threadIdx.x];
+        for (int q = 0; q < P2; ++q) {
+          const int s = tid + q * H;
+          const int sc = s < I::n3 ? s : 0;
+#pragma unroll
+          for (int k = 0; k < 9; ++k) jv[q][k] = geo.jinv[e * 9 * I::n3 + k * I::n3 + sc];
         }
       }
-    }
-    // chain-rule metrics of this thread's solution points: issued now, consumed after the gradient DMMAs
-    double jv[P2][9];
-    if (GRADV != 0) {
+      bar_sync(kBarIn, kMainThreads);          // inputs and wall states are in shared memory
+      CHORUS_TICK(1);
+      // ---- A3: BR1 gradient.  d/dxi_d by DMMA, then the chain rule per point.
+      if constexpr (GRADV != 0) {
+        if (active) {
 #pragma unroll
-      for (int q = 0; q < P2; ++q) {
-        const int s = threadIdx.x + q * M::kThreads;
-        const int sc = s < I::n3 ? s : 0;
-#pragma unroll
-        for (int k = 0; k < 9; ++k) jv[q][k] = geo.jinv[e * 9 * I::n3 + k * I::n3 + sc];
-      }
-    }
-    cp_async_wait_all();
-    __syncthreads();
-    CHORUS_TICK(1);
-    for (int t = threadIdx.x; t < 6 * I::n2; t += blockDim.x) {     // wall faces: the boundary state Q_b takes the neighbour's place
-      const int f = t / I::n2, ab = t % I::n2;
-      const int ne = nb.ne[f];
-      if (ne < 0) {
-        double own[9], out[9];
-#pragma unroll
-        for (int v = 0; v < 9; ++v) own[v] = sQo[(f * 9 + v) * I::n2 + ab];
-        const double* nf_ = geo.nfc + ((e * 6 + f) * 4) * I::n2 + ab;
-        wall_state(ph, ne, own, nf_[0], nf_[I::n2], nf_[2 * I::n2], out);
-#pragma unroll
-        for (int v = 0; v < 9; ++v) sQn[(f * 9 + v) * I::n2 + ab] = out[v];
-      }
-    }
-    __syncthreads();
-    CHORUS_TICK(2);
-
-    // ---- A3: BR1 gradient.  d/dxi_d by DMMA (warp = line group, all directions), then the chain rule per point.
-    if constexpr (GRADV != 0) {
-#pragma unroll
-      for (int k = 0; k < M::kTPD; ++k)
-        if (warp + k * M::kWarps < M::FG) {
-          grad_dir<N, NGV, GV0, 0>(L, nb, sQ, sQo, sQn, sG, lnd[0][k], true);
-          grad_dir<N, NGV, GV0, 1>(L, nb, sQ, sQo, sQn, sG, lnd[1][k], true);
-          grad_dir<N, NGV, GV0, 2>(L, nb, sQ, sQo, sQn, sG, lnd[2][k], true);
-        }
-      if (M::kTail > 0 && tw < M::kTail) grad_dir<N, NGV, GV0, 3>(L, nb, sQ, sQo, sQn, sG, tl_ln, tl_ok, tl_d);
-      __syncthreads();
-      CHORUS_TICK(3);
-#pragma unroll
-      for (int q = 0; q < P2; ++q) {
-        const int s = threadIdx.x + q * M::kThreads;
-        if (s < I::n3) {
-#pragma unroll
-          for (int vv = 0; vv < NGV; ++vv) {
-            const double g0 = sG[(vv * 3 + 0) * I::n3 + s], g1 = sG[(vv * 3 + 1) * I::n3 + s], g2 = sG[(vv * 3 + 2) * I::n3 + s];
-#pragma unroll
-            for (int p = 0; p < 3; ++p) sG[(vv * 3 + p) * I::n3 + s] = jv[q][p] * g0 + jv[q][3 + p] * g1 + jv[q][6 + p] * g2;
-          }
+          for (int k = 0; k < M::kTPD; ++k)
+            if (warp + k * M::kWarps < M::FG) {
+              grad_dir<N, NGV, GV0, 0>(L, nb, sQ, sQo, sQn, sG, lnd[0][k], true);
+              grad_dir<N, NGV, GV0, 1>(L, nb, sQ, sQo, sQn, sG, lnd[1][k], true);
+              grad_dir<N, NGV, GV0, 2>(L, nb, sQ, sQo, sQn, sG, lnd[2][k], true);
+            }
+          if (M::kTail > 0 && tw < M::kTail) grad_dir<N, NGV, GV0, 3>(L, nb, sQ, sQo, sQn, sG, tl_ln, tl_ok, tl_d);
         }
       }
-    }
-    CHORUS_TICK(4);
-
-    // ---- A6: common INVISCID fluxes at the 6 n^2 face points (Rusanov / wall), scaled by sigma |S|, in place over sQn
-    {
-      double nq[F2][4];
+      bar_sync(kBarGrad, kMainThreads);        // gradient DMMAs done (the helpers hold the face fluxes in registers)
+      CHORUS_TICK(2);
+      if constexpr (GRADV != 0) {
 #pragma unroll
-      for (int q = 0; q < F2; ++q) {
-        const int t = threadIdx.x + q * M::kThreads;
-        const int tc = t < 6 * I::n2 ? t : 0;
-        const double* nf_ = geo.nfc + (e * 6 + tc / I::n2) * 4 * I::n2 + tc % I::n2;
+        for (int q = 0; q < P2; ++q) {
+          const int s = tid + q * H;
+          if (s < I::n3) {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) nq[q][k] = nf_[k * I::n2];
-      }
+            for (int vv = 0; vv < NGV; ++vv) {
+              const double g0 = sG[(vv * 3 + 0) * I::n3 + s], g1 = sG[(vv * 3 + 1) * I::n3 + s], g2 = sG[(vv * 3 + 2) * I::n3 + s];
 #pragma unroll
-      for (int q = 0; q < F2; ++q) {
-        const int t = threadIdx.x + q * M::kThreads;
-        if (t < 6 * I::n2) {
-          const int f = t / I::n2, ab = t % I::n2;
-          double Qo[9], F[9];
-#pragma unroll
-          for (int v = 0; v < 9; ++v) Qo[v] = sQn[(f * 9 + v) * I::n2 + ab];
-          if (nb.ne[f] >= 0) {
-            double Qi[9];
-#pragma unroll
-            for (int v = 0; v < 9; ++v) Qi[v] = sQo[(f * 9 + v) * I::n2 + ab];
-            flux_rusanov(ph, Qi, Qo, nq[q][0], nq[q][1], nq[q][2], F);
-          } else {
-            const PrimD sb_ = primitives(ph, Qo);          // Qo holds the wall state Q_b
-            flux_inviscid<true>(ph, sb_, nq[q][0], nq[q][1], nq[q][2], F);
-          }
-#pragma unroll
-          for (int v = 0; v < 9; ++v) sQn[(f * 9 + v) * I::n2 + ab] = nq[q][3] * F[v];
-        }
-      }
-    }
-#ifdef CHORUS_L2_PREFETCH
-    if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, 2);
-#endif
-    __syncthreads();              // own traces (sQo) are dead from here on: the region becomes sR
-    CHORUS_TICK(5);
-
-    // ---- A1, A4, A5, A7: one DMMA chain per warp and direction.  Direction 0 stores into sR, the others accumulate, so the
-    //      directions are separated by barriers; the points of the left-over direction-0 lines start from zero.
-    if (M::LO > 0) {
-      for (int t = threadIdx.x; t < 9 * M::LO * N; t += blockDim.x) {
-        const int l = t % N, i = (t / N) % M::LO, v = t / (N * M::LO);
-        sR[v * I::n3 + I::sbase(0, M::line_of(0, 8 * M::FG + i)) + l] = 0.0;
-      }
-    }
-#pragma unroll
-    for (int k = 0; k < M::kTPD; ++k)
-      if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 0>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[0][k], true);
-#ifdef CHORUS_L2_PREFETCH
-    if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, 0);
-#endif
-    __syncthreads();
-    CHORUS_TICK(6);
-#pragma unroll
-    for (int k = 0; k < M::kTPD; ++k)
-      if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
-#ifdef CHORUS_L2_PREFETCH
-    if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, 1);
-#endif
-    __syncthreads();
-    CHORUS_TICK(7);
-    // epilogue inputs of this thread's solution points: issued before the last chain, consumed after it
-    double ej[P2], ex[P2][3];
-#pragma unroll
-    for (int q = 0; q < P2; ++q) {
-      const int s = threadIdx.x + q * M::kThreads;
-      const int sc = s < I::n3 ? s : 0;
-      ej[q] = geo.detJ[e * I::n3 + sc];
-#pragma unroll
-      for (int k = 0; k < 3; ++k) ex[q][k] = geo.xsol[(e * 3 + k) * I::n3 + sc];
-    }
-#pragma unroll
-    for (int k = 0; k < M::kTPD; ++k)
-      if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
-    __syncthreads();
-    if (M::kTail > 0) {   // left-over lines of the three directions: no two of them share a solution point
-      if (tw < M::kTail) chain_dir<N, DIFF, 3>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, tl_ln, tl_ok, tl_d);
-      __syncthreads();
-    }
-    CHORUS_TICK(8);
-
-    // ---- A8 + A9
-    {
-      const bool rk = io.Qout != nullptr;
-      const bool g0 = rk && io.A0 != nullptr, g1 = rk && io.A1 != nullptr;
-      double a0[P2][9], a1[P2][9];     // stage registers read from HBM: all loads in flight before any use
-#pragma unroll
-      for (int q = 0; q < P2; ++q) {
-        const int s = threadIdx.x + q * M::kThreads;
-        const int sc = s < I::n3 ? s : 0;
-#pragma unroll
-        for (int v = 0; v < 9; ++v) {
-          const int64_t ix = (e * 9 + v) * I::n3 + sc;
-          a0[q][v] = g0 ? io.A0[ix] : 0.0;
-          a1[q][v] = g1 ? io.A1[ix] : 0.0;
-        }
-      }
-#pragma unroll
-      for (int q = 0; q < P2; ++q) {
-        const int s = threadIdx.x + q * M::kThreads;
-        if (s < I::n3) {
-          double Q[9], R[9];
-#pragma unroll
-          for (int v = 0; v < 9; ++v) Q[v] = sQ[v * I::n3 + s];
-          const double rj = -1.0 / ej[q];
-#pragma unroll
-          for (int v = 0; v < 9; ++v) R[v] = sR[v * I::n3 + s] * rj;
-          double divB = 0.0;
-          if (GRADV == 2) divB = sG[15 * I::n3 + s] + sG[19 * I::n3 + s] + sG[23 * I::n3 + s];
-          if (GRADV == 1) divB = sG[0 * I::n3 + s] + sG[4 * I::n3 + s] + sG[8 * I::n3 + s];
-          const PrimD p = primitives(ph, Q);
-          add_sources(ph, p, divB, ex[q][0], ex[q][1], ex[q][2], R);
-          if (rk) {                      // step mode: Runge-Kutta combination
-#pragma unroll
-            for (int v = 0; v < 9; ++v) {
-              R[v] = io.bdt * R[v] + io.c0 * a0[q][v] + io.c1 * a1[q][v] + io.cq * Q[v];
+              for (int p = 0; p < 3; ++p) sG[(vv * 3 + p) * I::n3 + s] = jv[q][p] * g0 + jv[q][3 + p] * g1 + jv[q][6 + p] * g2;
             }
           }
+        }
+      }
+      bar_sync(kBarChain, H);                  // the gradient is complete in shared memory
+      CHORUS_TICK(3);
+      // ---- A1, A4, A5, A7: one DMMA chain per warp and direction, directions separated by chain-warp barriers
+      if (active) {
+        chain_dir<N, DIFF, 0, true>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[0][0], true, 0, tid);
+#pragma unroll
+        for (int k = 1; k < M::kTPD; ++k)
+          if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 0>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[0][k], true);
+      } else {
+        bar_sync(kBarFaces, kMainThreads);
+      }
+      bar_sync(kBarChain, H);
+      CHORUS_TICK(4);
+      if (active) {
+#pragma unroll
+        for (int k = 0; k < M::kTPD; ++k)
+          if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
+      }
+      bar_sync(kBarChain, H);
+      CHORUS_TICK(5);
+      if (active) {
+#pragma unroll
+        for (int k = 0; k < M::kTPD; ++k)
+          if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
+      }
+      if (M::kTail > 0) {   // left-over lines of the three directions: no two of them share a solution point
+        bar_sync(kBarChain, H);
+        CHORUS_TICK(6);
+        if (active && tw < M::kTail) chain_dir<N, DIFF, 3>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, tl_ln, tl_ok, tl_d);
+      }
+      bar_sync(kBarRes, kMainThreads);         // divergence accumulated: the helpers finish the element
+      CHORUS_TICK(7);
+    }
+  } else {
+    // =============================================== helper warps ==============================================
+    setmaxnreg_dec<kHelpRegs>();
+    constexpr bool kVec = (9 * I::n3) % 2 == 0 && (54 * I::n2) % 2 == 0;     // 16-byte cp.async possible for the state and the traces
+    constexpr int P2 = (I::n3 + H - 1) / H;              // solution points per helper thread
+    // connectivity of the element this CTA handles next, fetched one element ahead by helper threads 0..5
+    int pn_e = 0, pn_f = 0, pn_o = 0;
+    auto fetch_nbr = [&](int64_t el) {
+      if (tid < 6 && el < E) {
+        pn_e = geo.nbr_elem[el * 6 + tid];
+        pn_f = geo.nbr_face[el * 6 + tid];
+        pn_o = geo.nbr_orient[el * 6 + tid];
+      }
+    };
+    // asynchronous load of one element's inputs: state, own traces, S^d, neighbour traces through the orientation map (A2)
+    // part A: state, S^d and neighbour traces (their shared memory is dead as soon as the chains are done);
+    // part B: own traces (their region doubles as the divergence accumulator sR, read by the final combination)
+    auto issue_loads_a = [&](int64_t el) {
+      if (tid < 6) { nb.ne[tid] = pn_e; nb.nf[tid] = pn_f; nb.no[tid] = pn_o; }
+      const double* q = io.Qe + el * 9 * I::n3;
+      const double* g = geo.Sfl + el * 9 * I::nf;
+      if (kVec) {
+        for (int k = tid; k < 9 * I::n3 / 2; k += H) cp_async16(sQ + 2 * k, q + 2 * k);
+      } else {
+        for (int k = tid; k < 9 * I::n3; k += H) cp_async8(sQ + k, q + k);
+      }
+      for (int k = tid; k < 9 * I::nf / 2; k += H) cp_async16(sS + 2 * k, g + 2 * k);
+      bar_sync(kBarHelp, H);   // nb visible
+      for (int k = tid; k < 6 * I::n2; k += H) {
+        const int f = k / I::n2, ab = k % I::n2;
+        const int ne = nb.ne[f];
+        if (ne >= 0) {
+          const double* src = io.Qf + (((int64_t)ne * 6 + nb.nf[f]) * 9) * I::n2 + I::orient(nb.no[f], ab);
+#pragma unroll
+          for (int v = 0; v < 9; ++v) cp_async8(sQn + (f * 9 + v) * I::n2 + ab, src + v * I::n2);
+        }
+      }
+    };
+    auto issue_loads_b = [&](int64_t el) {
+      const double* t = io.Qf + el * 54 * I::n2;
+      if (kVec) {
+        for (int k = tid; k < 54 * I::n2 / 2; k += H) cp_async16(sQo + 2 * k, t + 2 * k);
+      } else {
+        for (int k = tid; k < 54 * I::n2; k += H) cp_async8(sQo + k, t + k);
+      }
+      cp_async_commit();
+    };
+    fetch_nbr(blockIdx.x);
+    if ((int64_t)blockIdx.x < E) {
+      issue_loads_a(blockIdx.x);
+      issue_loads_b(blockIdx.x);
+      fetch_nbr((int64_t)blockIdx.x + gridDim.x);
+    }
+    const bool rk = io.Qout != nullptr;
+    const bool g0 = rk && io.A0 != nullptr, g1 = rk && io.A1 != nullptr;
+
+    for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
+      cp_async_wait_all();
+      bar_sync(kBarHelp, H);                   // every helper's copies have landed
+      for (int t = tid; t < 6 * I::n2; t += H) {     // wall faces: the boundary state Q_b takes the neighbour's place
+        const int f = t / I::n2, ab = t % I::n2;
+        const int ne = nb.ne[f];
+        if (ne < 0) {
+          double own[9], out[9];
+#pragma unroll
+          for (int v = 0; v < 9; ++v) own[v] = sQo[(f * 9 + v) * I::n2 + ab];
+          const double* nf_ = geo.nfc + ((e * 6 + f) * 4) * I::n2 + ab;
+          wall_state(ph, ne, own, nf_[0], nf_[I::n2], nf_[2 * I::n2], out);
+#pragma unroll
+          for (int v = 0; v < 9; ++v) sQn[(f * 9 + v) * I::n2 + ab] = out[v];
+        }
+      }
+      bar_sync(kBarIn, kMainThreads);
+
+      // ---- A6: common INVISCID fluxes at the 6 n^2 face points (Rusanov / wall), scaled by sigma |S|.  They replace the
+      //      neighbour traces in sQn, which the gradient is still reading: computed now, stored after the GRAD barrier.
+      auto face_flux = [&](int t, double* F) {
+        const int f = t / I::n2, ab = t % I::n2;
+        const double* nf_ = geo.nfc + (e * 6 + f) * 4 * I::n2 + ab;
+        const double nx = nf_[0], ny = nf_[I::n2], nz = nf_[2 * I::n2], sa = nf_[3 * I::n2];
+        double Qo[9];
+#pragma unroll
+        for (int v = 0; v < 9; ++v) Qo[v] = sQn[(f * 9 + v) * I::n2 + ab];
+        if (nb.ne[f] >= 0) {
+          double Qi[9];
+#pragma unroll
+          for (int v = 0; v < 9; ++v) Qi[v] = sQo[(f * 9 + v) * I::n2 + ab];
+          flux_rusanov(ph, Qi, Qo, nx, ny, nz, F);
+        } else {
+          const PrimD sb_ = primitives(ph, Qo);          // Qo holds the wall state Q_b
+          flux_inviscid<true>(ph, sb_, nx, ny, nz, F);
+        }
+#pragma unroll
+        for (int v = 0; v < 9; ++v) F[v] *= sa;
+      };
+      {
+        double Ff[9];                              // one face point per helper thread beside the gradient DMMAs ...
+        if (tid < 6 * I::n2) face_flux(tid, Ff);
+        bar_sync(kBarGrad, kMainThreads);
+        if (tid < 6 * I::n2) {
+          const int f = tid / I::n2, ab = tid % I::n2;
+#pragma unroll
+          for (int v = 0; v < 9; ++v) sQn[(f * 9 + v) * I::n2 + ab] = Ff[v];
+        }
+        for (int t = tid + H; t < 6 * I::n2; t += H) {   // ... the rest beside the chain rule, in place (own face point only)
+          double F[9];
+          face_flux(t, F);
+          const int f = t / I::n2, ab = t % I::n2;
+#pragma unroll
+          for (int v = 0; v < 9; ++v) sQn[(f * 9 + v) * I::n2 + ab] = F[v];
+        }
+      }
+      bar_sync(kBarFaces, kMainThreads);
+
+      // ---- beside the chains: A8 sources and the Runge-Kutta registers, so that  out = w * sR + K  is all that is left
+      double K[P2][9], w[P2];
+#pragma unroll
+      for (int q = 0; q < P2; ++q) {
+        const int s = tid + q * H;
+        const int sc = s < I::n3 ? s : 0;
+        double Q[9];
+#pragma unroll
+        for (int v = 0; v < 9; ++v) Q[v] = sQ[v * I::n3 + sc];
+        double divB = 0.0;
+        if (GRADV == 2) divB = sG[15 * I::n3 + sc] + sG[19 * I::n3 + sc] + sG[23 * I::n3 + sc];
+        if (GRADV == 1) divB = sG[0 * I::n3 + sc] + sG[4 * I::n3 + sc] + sG[8 * I::n3 + sc];
+        {
+          const PrimD p = primitives(ph, Q);
+#pragma unroll
+          for (int v = 0; v < 9; ++v) K[q][v] = 0.0;
+          add_sources(ph, p, divB, geo.xsol[(e * 3 + 0) * I::n3 + sc], geo.xsol[(e * 3 + 1) * I::n3 + sc],
+                      geo.xsol[(e * 3 + 2) * I::n3 + sc], K[q]);                                      // K = M (Eq. 5)
+        }
+        w[q] = -1.0 / geo.detJ[e * I::n3 + sc];              // R = w * div_xi F~ + M  (Eq. 16)
+        if (rk) {                                            // step mode: out = cq Q + c0 A0 + c1 A1 + bdt R
+          w[q] *= io.bdt;
+#pragma unroll
+          for (int v = 0; v < 9; ++v) K[q][v] = io.bdt * K[q][v] + io.cq * Q[v];
+          if (g0) {
+#pragma unroll
+            for (int v = 0; v < 9; ++v) K[q][v] += io.c0 * io.A0[(e * 9 + v) * I::n3 + sc];
+          }
+          if (g1) {
+#pragma unroll
+            for (int v = 0; v < 9; ++v) K[q][v] += io.c1 * io.A1[(e * 9 + v) * I::n3 + sc];
+          }
+        }
+      }
+#ifndef CHORUS_NO_L2_PREFETCH   // measured: -0.9k cycles of the 6.2k the chain warps wait for the next element's inputs
+      if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, pn_e, pn_f, tid, H);
+#endif
+      bar_sync(kBarRes, kMainThreads);
+
+      // ---- A9: finish the element.  The next element's state, metrics and neighbour traces start streaming in first
+      //      (except when this element's new state still has to pass through sQ for its traces)
+      constexpr bool kEarlyLoads = DIFF;
+      const bool more = e + gridDim.x < E;
+      if (kEarlyLoads && more) issue_loads_a(e + gridDim.x);
+#pragma unroll
+      for (int q = 0; q < P2; ++q) {
+        const int s = tid + q * H;
+        if (s < I::n3) {
+          double R[9];
+#pragma unroll
+          for (int v = 0; v < 9; ++v) R[v] = w[q] * sR[v * I::n3 + s] + K[q][v];
           if (DIFF) {                    // finished by the face kernel
 #pragma unroll
             for (int v = 0; v < 9; ++v) io.Part[(e * 9 + v) * I::n3 + s] = R[v];
@@ -842,12 +926,17 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           }
         }
       }
+      if (!DIFF && rk) {
+        bar_sync(kBarHelp, H);
+        emit_traces<N>(sQ, io.QfOut + e * 54 * I::n2, tid, H);
+      }
+      bar_sync(kBarHelp, H);                   // every helper is done with this element's shared memory
+      if (more) {
+        if (!kEarlyLoads) issue_loads_a(e + gridDim.x);
+        issue_loads_b(e + gridDim.x);
+        fetch_nbr(e + 2 * (int64_t)gridDim.x);
+      }
     }
-    if (!DIFF && io.Qout != nullptr) {
-      __syncthreads();
-      emit_traces<N>(sQ, io.QfOut + e * 54 * I::n2);
-    }
-    CHORUS_TICK(9);
   }
 }
 
@@ -922,7 +1011,7 @@ __global__ void __launch_bounds__(256) stage_face_kernel(int64_t E, StageIO io, 
     }
     if (step) {
       __syncthreads();
-      emit_traces<N>(sP, io.QfOut + e * 54 * I::n2);
+      emit_traces<N>(sP, io.QfOut + e * 54 * I::n2, threadIdx.x, blockDim.x);
     }
   }
 }

@@ -18,7 +18,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def test_header_and_library_symbols_match():
     hdr = open(os.path.join(ROOT, "include", "chorus.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(chorus_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(chorus_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(P.SYMBOLS)
     L = P.lib()
     for s in P.SYMBOLS:

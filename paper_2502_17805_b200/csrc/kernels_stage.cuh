@@ -253,6 +253,39 @@ __device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
+// ---- TMA (bulk asynchronous copy, SASS UBLKCP) with mbarrier completion
+__device__ __forceinline__ void mbar_init(uint64_t* mb, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(mb)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* mb, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(mb)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* mb, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"((unsigned)__cvta_generic_to_shared(mb)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load(void* smem, const void* gmem, unsigned bytes, uint64_t* mb) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(smem)),
+               "l"(gmem), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(mb))
+               : "memory");
+}
+// Not needed on the load path: every generic-proxy access to a destination buffer has been performed and observed by other
+// threads (barrier-ordered) before the bulk copy that overwrites it is issued -- the consumer-release -> producer-load pattern.
+// (Measured cost when issued by a thread with global stores in flight: ~1k cycles.)  -DCHORUS_PROXY_FENCE puts it back.
+__device__ __forceinline__ void fence_proxy_async() {
+#ifdef CHORUS_PROXY_FENCE
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+#endif
+}
+
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
 // all threads of the CTA: prefetch `bytes` starting at p into L2, one request per 128-byte line
 __device__ __forceinline__ void prefetch_block_l2(const void* p, size_t bytes, int tid, int nthreads) {
@@ -590,13 +623,19 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   double* sR = sQo;
   __shared__ ElemNbr nb;
   __shared__ int s_second;
+  __shared__ __align__(8) uint64_t mbar;   // completion of the bulk (TMA) copies of one element
   if (threadIdx.x == 0) {
     unsigned smid;
     asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
     s_second = (int)(atomicAdd(io.sm_arrivals + smid, 1u) & 1u);
+    mbar_init(&mbar, 2);     // two producer arrivals per element: part A and part B of its loads
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   __syncthreads();
   const int wg = threadIdx.x >> 7, tid = threadIdx.x & 127;
+  // The contiguous per-element blocks (state, own traces, S^d) go by TMA bulk copy when they are 16-byte aligned (n even);
+  // the neighbour traces are gathered through the orientation map with 8-byte cp.async either way.
+  constexpr bool kBulk = (9 * I::n3) % 2 == 0 && (54 * I::n2) % 2 == 0;
   constexpr int H = 128;                 // threads per warpgroup
 
   if (wg == 0) {
@@ -659,6 +698,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
 #ifdef CHORUS_PHASE_TIMING
     long long tick_ = clock64();
 #endif
+    unsigned ld_phase = 0;
     for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
       CHORUS_TICK(0);
       int tw = M::kWarps, tl_d = 0, tl_ln = 0;
@@ -682,6 +722,8 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           for (int k = 0; k < 9; ++k) jv[q][k] = geo.jinv[e * 9 * I::n3 + k * I::n3 + sc];
         }
       }
+      if (kBulk) mbar_wait(&mbar, ld_phase);   // bulk copies: completion is observed by every consumer thread itself
+      ld_phase ^= 1u;
       bar_sync(kBarIn, kMainThreads);          // inputs and wall states are in shared memory
       CHORUS_TICK(1);
       // ---- A3: BR1 gradient.  d/dxi_d by DMMA, then the chain rule per point.
@@ -749,7 +791,6 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   } else {
     // =============================================== helper warps ==============================================
     setmaxnreg_dec<kHelpRegs>();
-    constexpr bool kVec = (9 * I::n3) % 2 == 0 && (54 * I::n2) % 2 == 0;     // 16-byte cp.async possible for the state and the traces
     constexpr int P2 = (I::n3 + H - 1) / H;              // solution points per helper thread
     // connectivity of the element this CTA handles next, fetched one element ahead by helper threads 0..5
     int pn_e = 0, pn_f = 0, pn_o = 0;
@@ -767,12 +808,17 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       if (tid < 6) { nb.ne[tid] = pn_e; nb.nf[tid] = pn_f; nb.no[tid] = pn_o; }
       const double* q = io.Qe + el * 9 * I::n3;
       const double* g = geo.Sfl + el * 9 * I::nf;
-      if (kVec) {
-        for (int k = tid; k < 9 * I::n3 / 2; k += H) cp_async16(sQ + 2 * k, q + 2 * k);
+      if (kBulk) {
+        if (tid == 0) {
+          mbar_expect_tx(&mbar, (unsigned)(sizeof(double) * (9 * I::n3 + 9 * I::nf)));
+          tma_load(sQ, q, sizeof(double) * 9 * I::n3, &mbar);
+        } else if (tid == 32) {
+          tma_load(sS, g, sizeof(double) * 9 * I::nf, &mbar);
+        }
       } else {
         for (int k = tid; k < 9 * I::n3; k += H) cp_async8(sQ + k, q + k);
+        for (int k = tid; k < 9 * I::nf / 2; k += H) cp_async16(sS + 2 * k, g + 2 * k);
       }
-      for (int k = tid; k < 9 * I::nf / 2; k += H) cp_async16(sS + 2 * k, g + 2 * k);
       bar_sync(kBarHelp, H);   // nb visible
       for (int k = tid; k < 6 * I::n2; k += H) {
         const int f = k / I::n2, ab = k % I::n2;
@@ -786,8 +832,11 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     };
     auto issue_loads_b = [&](int64_t el) {
       const double* t = io.Qf + el * 54 * I::n2;
-      if (kVec) {
-        for (int k = tid; k < 54 * I::n2 / 2; k += H) cp_async16(sQo + 2 * k, t + 2 * k);
+      if (kBulk) {
+        if (tid == 64) {
+          mbar_expect_tx(&mbar, (unsigned)(sizeof(double) * 54 * I::n2));
+          tma_load(sQo, t, sizeof(double) * 54 * I::n2, &mbar);
+        }
       } else {
         for (int k = tid; k < 54 * I::n2; k += H) cp_async8(sQo + k, t + k);
       }
@@ -802,9 +851,12 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     const bool rk = io.Qout != nullptr;
     const bool g0 = rk && io.A0 != nullptr, g1 = rk && io.A1 != nullptr;
 
+    unsigned ld_phase = 0;
     for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
       cp_async_wait_all();
-      bar_sync(kBarHelp, H);                   // every helper's copies have landed
+      if (kBulk) mbar_wait(&mbar, ld_phase);   // the bulk copies have landed ...
+      ld_phase ^= 1u;
+      bar_sync(kBarHelp, H);                   // ... and every helper's gathered copies
       for (int t = tid; t < 6 * I::n2; t += H) {     // wall faces: the boundary state Q_b takes the neighbour's place
         const int f = t / I::n2, ab = t % I::n2;
         const int ne = nb.ne[f];

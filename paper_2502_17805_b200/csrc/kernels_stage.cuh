@@ -809,9 +809,16 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       const double* q = io.Qe + el * 9 * I::n3;
       const double* g = geo.Sfl + el * 9 * I::nf;
       if (kBulk) {
-        if (tid == 0) {
-          mbar_expect_tx(&mbar, (unsigned)(sizeof(double) * (9 * I::n3 + 9 * I::nf)));
-          tma_load(sQ, q, sizeof(double) * 9 * I::n3, &mbar);
+        if (tid < 32) {
+          // neighbour faces that meet this element with the identity orientation (all faces inside a panel, most seam faces)
+          // are contiguous 9 n^2 blocks in the same indexing: one bulk copy each, issued by the thread that holds the face
+          const bool whole = tid < 6 && pn_e >= 0 && pn_o == 0;
+          const unsigned cnt = __popc(__ballot_sync(0xffffffffu, whole));
+          if (tid == 0) {
+            mbar_expect_tx(&mbar, (unsigned)(sizeof(double) * (9 * I::n3 + 9 * I::nf + cnt * 9 * I::n2)));
+            tma_load(sQ, q, sizeof(double) * 9 * I::n3, &mbar);
+          }
+          if (whole) tma_load(sQn + tid * 9 * I::n2, io.Qf + ((int64_t)pn_e * 6 + pn_f) * 9 * I::n2, sizeof(double) * 9 * I::n2, &mbar);
         } else if (tid == 32) {
           tma_load(sS, g, sizeof(double) * 9 * I::nf, &mbar);
         }
@@ -823,7 +830,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       for (int k = tid; k < 6 * I::n2; k += H) {
         const int f = k / I::n2, ab = k % I::n2;
         const int ne = nb.ne[f];
-        if (ne >= 0) {
+        if (ne >= 0 && !(kBulk && nb.no[f] == 0)) {     // the other orientations: gathered point by point
           const double* src = io.Qf + (((int64_t)ne * 6 + nb.nf[f]) * 9) * I::n2 + I::orient(nb.no[f], ab);
 #pragma unroll
           for (int v = 0; v < 9; ++v) cp_async8(sQn + (f * 9 + v) * I::n2 + ab, src + v * I::n2);

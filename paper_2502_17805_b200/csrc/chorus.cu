@@ -129,8 +129,7 @@ struct Hot {
   template <bool DIFF, int GRADV>
   static int main_launch(chorus_ctx* c, const StageIO& io) {
     if constexpr (N >= 4 && N <= 7) {
-      size_t smem = stage_main_smem_bytes<N, GRADV>();
-      if (std::getenv("CHORUS_ONE_CTA")) smem = c->max_smem - 1024;   // experiment: one CTA per SM
+      constexpr size_t smem = stage_main_smem_bytes<N, GRADV>();
       constexpr int threads = kMainThreads;
       auto k = stage_main_kernel<N, DIFF, GRADV>;
       CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

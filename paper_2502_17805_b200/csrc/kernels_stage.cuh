@@ -42,7 +42,6 @@ struct Mma {
   // would double the load of one FP64 pipe (measured: 5 warps of DMMA take twice as long as 4).
   static constexpr int FG = I::n2 / 8, LO = I::n2 % 8;
   static constexpr int kWarps = FG < 4 ? FG : 4;
-  static constexpr int kThreads = 32 * kWarps;
   static constexpr int kTPD = (FG + kWarps - 1) / kWarps;     // directional tasks per warp and direction
   static constexpr int kTail = (3 * LO + 7) / 8;               // tail tasks per element
   static_assert(kTail <= kWarps, "tail tasks: one round");
@@ -122,36 +121,6 @@ __device__ __forceinline__ void emit_traces(const double* sQ, double* __restrict
     }
     Qf_e[((2 * d) * 9 + v) * I::n2 + ab] = lo;
     Qf_e[((2 * d + 1) * 9 + v) * I::n2 + ab] = hi;
-  }
-}
-
-// Stage the own traces and the neighbours' traces of one element in shared memory (A2, walls :190-198).
-//   sQo[f][v][ab] = own polynomial at the face point;  sQn[f][v][ab] = neighbour's polynomial there, or, on a wall face,
-//   the boundary state Q_b (so that "common solution" = Q_b and "outer state" = Q_b both read sQn).
-template <int N>
-__device__ __forceinline__ void stage_traces_n(int64_t e, const ElemNbr& nb, const PhysD& ph, const double* __restrict__ Qf,
-                                               const double* __restrict__ nfc, double* sQo, double* sQn) {
-  using I = Ix<N>;
-  for (int t = threadIdx.x; t < 6 * I::n2; t += blockDim.x) {
-    const int f = t / I::n2, ab = t % I::n2;
-    double own[9], out[9];
-#pragma unroll
-    for (int v = 0; v < 9; ++v) own[v] = Qf[((e * 6 + f) * 9 + v) * I::n2 + ab];
-    const int ne = nb.ne[f];
-    if (ne >= 0) {
-      const int ab2 = I::orient(nb.no[f], ab);
-      const double* src = Qf + (((int64_t)ne * 6 + nb.nf[f]) * 9) * I::n2 + ab2;
-#pragma unroll
-      for (int v = 0; v < 9; ++v) out[v] = src[v * I::n2];
-    } else {
-      const double* nf_ = nfc + ((e * 6 + f) * 4) * I::n2 + ab;
-      wall_state(ph, ne, own, nf_[0], nf_[I::n2], nf_[2 * I::n2], out);
-    }
-#pragma unroll
-    for (int v = 0; v < 9; ++v) {
-      sQo[(f * 9 + v) * I::n2 + ab] = own[v];
-      sQn[(f * 9 + v) * I::n2 + ab] = out[v];
-    }
   }
 }
 
@@ -308,7 +277,6 @@ constexpr int kChainRegs = 160, kHelpRegs = 96;   // 128 * (160 + 96) = the CTA'
 template <int N>
 struct LaneK {
   double bI0, bI1;     // interpolation operand, k-steps 0 and 1
-  double t0[2], t1[2]; // orders 5, 6: h_l(X_f) of l = 4, 5 at this thread's two columns (the short second k-step is done with DFMA)
   double bD0, bD1;     // derivative operand
   double bG[3];        // BR1 gradient operand
   int m0, m1;          // flux point of the two columns this thread holds (-1 = padding)
@@ -391,21 +359,7 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
   double q0[9], q1[9];
 #pragma unroll
   for (int v = 0; v < 9; ++v) dmma884z(q0[v], q1[v], A0[v * I::n3], L.bI0);
-  // second k-step (l = 4 .. N-1).  Orders 5 and 6 have only one or two terms left: four DFMA (8 pipe cycles) instead of a
-  // three-quarters-empty DMMA (16 pipe cycles); every thread of a row reads the same two values (broadcast).
-  constexpr bool kScalarTail = false;   // tried for N = 5, 6: fewer pipe cycles, but the extra live registers spill at 160 and the chains get slower
-  const double* T4 = sQ + sb + 4 * st;           // solution value l = 4 of this thread's line (l = 5: + st)
-  if (kScalarTail) {
-#pragma unroll
-    for (int v = 0; v < 9; ++v) {
-      const double x4 = T4[v * I::n3];
-      q0[v] = fma(x4, L.t0[0], q0[v]); q1[v] = fma(x4, L.t1[0], q1[v]);
-      if (N == 6) {
-        const double x5 = T4[v * I::n3 + st];
-        q0[v] = fma(x5, L.t0[1], q0[v]); q1[v] = fma(x5, L.t1[1], q1[v]);
-      }
-    }
-  } else if (N > 4) {
+  if (N > 4) {
 #pragma unroll
     for (int v = 0; v < 9; ++v) dmma884(q0[v], q1[v], A1[v * I::n3], L.bI1);
   }
@@ -460,25 +414,13 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
     VStream s0, s1;
     const double* G0 = sG + sb + c * st;
     const double* G1 = sG + sb + l1 * st;
-    const double* G4 = sG + sb + 4 * st;
 #define CHORUS_STREAM_VAR(V)                                             \
   {                                                                      \
     double ga0, ga1, gb0, gb1, gc0, gc1;                                   \
     dmma884z(ga0, ga1, G0[(3 * (V)) * I::n3], L.bI0);                    \
     dmma884z(gb0, gb1, G0[(3 * (V) + 1) * I::n3], L.bI0);                \
     dmma884z(gc0, gc1, G0[(3 * (V) + 2) * I::n3], L.bI0);                \
-    if (kScalarTail) {                                                   \
-      const double xa = G4[(3 * (V)) * I::n3], xb = G4[(3 * (V) + 1) * I::n3], xc = G4[(3 * (V) + 2) * I::n3]; \
-      ga0 = fma(xa, L.t0[0], ga0); ga1 = fma(xa, L.t1[0], ga1);          \
-      gb0 = fma(xb, L.t0[0], gb0); gb1 = fma(xb, L.t1[0], gb1);          \
-      gc0 = fma(xc, L.t0[0], gc0); gc1 = fma(xc, L.t1[0], gc1);          \
-      if (N == 6) {                                                      \
-        const double ya = G4[(3 * (V)) * I::n3 + st], yb = G4[(3 * (V) + 1) * I::n3 + st], yc = G4[(3 * (V) + 2) * I::n3 + st]; \
-        ga0 = fma(ya, L.t0[1], ga0); ga1 = fma(ya, L.t1[1], ga1);        \
-        gb0 = fma(yb, L.t0[1], gb0); gb1 = fma(yb, L.t1[1], gb1);        \
-        gc0 = fma(yc, L.t0[1], gc0); gc1 = fma(yc, L.t1[1], gc1);        \
-      }                                                                  \
-    } else if (N > 4) {                                                  \
+    if (N > 4) {                                                         \
       dmma884(ga0, ga1, G1[(3 * (V)) * I::n3], L.bI1);                   \
       dmma884(gb0, gb1, G1[(3 * (V) + 1) * I::n3], L.bI1);               \
       dmma884(gc0, gc1, G1[(3 * (V) + 2) * I::n3], L.bI1);               \
@@ -509,7 +451,7 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
     // Direction 0 stores into sR, the others accumulate; the points of the left-over direction-0 lines, which no direction-0
     // task touches, start from zero (they are first accumulated into after the next chain-warp barrier).
     using MM = Mma<N>;
-    if (MM::LO > 0) {
+    if constexpr (MM::LO > 0) {
       for (int t = ctid; t < 9 * MM::LO * N; t += 32 * MM::kWarps) {
         const int l = t % N, i = (t / N) % MM::LO, v = t / (N * MM::LO);
         sR[v * I::n3 + I::sbase(0, MM::line_of(0, 8 * MM::FG + i)) + l] = 0.0;
@@ -652,18 +594,12 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       // interpolation: B[k = l][n = col r] = h_l(X_f,m(r));  k-step s covers l = 4s + c
       const int mB = M::col_m(r);
       L.bI0 = 0.0; L.bI1 = 0.0;
-      L.t0[0] = L.t0[1] = L.t1[0] = L.t1[1] = 0.0;
       if (mB >= 0) {
         L.bI0 = op.Isf[mB * N + c];
         if (4 + c < N) L.bI1 = op.Isf[mB * N + 4 + c];
       }
       // derivative: B[k = col][n = l_out r] = l'_{m(col)}(X_s,l_out);  k-step s covers col = 2c + s  (the C -> A reuse)
       L.m0 = M::col_m(2 * c); L.m1 = M::col_m(2 * c + 1);
-#pragma unroll
-      for (int l = 4; l < N && l < 6; ++l) {
-        if (L.m0 >= 0) L.t0[l - 4] = op.Isf[L.m0 * N + l];
-        if (L.m1 >= 0) L.t1[l - 4] = op.Isf[L.m1 * N + l];
-      }
       L.bD0 = 0.0; L.bD1 = 0.0;
       if (r < N) {
         if (L.m0 >= 0) L.bD0 = op.Dfs[r * (N + 1) + L.m0];

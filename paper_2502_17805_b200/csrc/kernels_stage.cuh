@@ -156,18 +156,18 @@ __device__ __forceinline__ void vs_finish(const PhysD& ph, const VStream& s, con
   const double ir = p.ir;
   const double grS = Sx * s.gr0 + Sy * s.gr1 + Sz * s.gr2;
   const double uS = p.u * Sx + p.v * Sy + p.w * Sz;
-  const double mu = p.rho * ph.nu;
   const double divu = (s.divm - (p.u * s.gr0 + p.v * s.gr1 + p.w * s.gr2)) * ir;
-  const double lam = -(2.0 / 3.0) * mu * divu;                                     // Stokes
-  const double mi = mu * ir;
+  const double lam = -(2.0 / 3.0) * (p.rho * ph.nu) * divu;                        // Stokes; mu = rho nu (G11)
+  const double mi = ph.nu;                                                         // mu / rho
   t0 = mi * ((s.mS0 - p.u * grS) + (s.W0 - uS * s.gr0)) + lam * Sx;                // Eq. 8 contracted with S
   t1 = mi * ((s.mS1 - p.v * grS) + (s.W1 - uS * s.gr1)) + lam * Sy;
   t2 = mi * ((s.mS2 - p.w * grS) + (s.W2 - uS * s.gr2)) + lam * Sz;
   const double u2 = p.u * p.u + p.v * p.v + p.w * p.w;
   const double dpS = ph.gm1 * (s.acc - (p.u * s.mS0 + p.v * s.mS1 + p.w * s.mS2) + 0.5 * u2 * grS);
-  const double Tt = p.p * ir * ph.iR;
-  const double dTS = (dpS - p.p * ir * grS) * ir * ph.iR;
-  const double dSS = ph.Cp * (dpS * ph.igamma / p.p - grS * ir);                   // gradient of Eq. 10
+  const double pr = p.p * ir;                                                      // p / rho = R T
+  const double Tt = pr * ph.iR;
+  const double dTS = (dpS - pr * grS) * ir * ph.iR;
+  const double dSS = ph.Cp * (dpS * ph.igamma * (1.0 / p.p) - grS * ir);           // gradient of Eq. 10
   qS = -ph.kappa * p.rho * Tt * dSS - kr * p.rho * ph.Cp * dTS;                    // Eq. 9
 }
 

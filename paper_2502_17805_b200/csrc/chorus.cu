@@ -47,6 +47,8 @@ struct chorus_ctx {
   double* d_Vf = nullptr;
   unsigned long long* d_ws = nullptr;
   unsigned* d_arrivals = nullptr;   // per-SM CTA arrival counters of the main kernel
+  double* d_scratch = nullptr;      // per-CTA global scratch of the scalar kernels' SPILL variants (orders 8, 9 with diffusion)
+  size_t scratch_doubles = 0;
   int64_t launches = 0;
   bool use_mma = true;   // orders 4..7: two-kernel DMMA pipeline (kernels_stage.cuh); CHORUS_KERNELS=scalar selects the
                          // three-kernel shared-memory path that serves the other orders (kernels_residual.cuh)
@@ -103,27 +105,46 @@ int gradv_of(const chorus_physics& p) { return (p.flags & kFlagDiffusion) ? 2 : 
 template <int N>
 struct Hot {
   using I = Ix<N>;
-  template <bool DIFF, int GRADV>
-  static int residual_launch(chorus_ctx* c, const double* Qin, const StageOut& out) {
-    constexpr size_t smem = residual_smem_bytes<N, DIFF, GRADV>();
+  // per-CTA global scratch for the SPILL variants of the scalar kernels (orders whose tiles exceed shared memory)
+  static int need_scratch(chorus_ctx* c, size_t doubles) {
+    if (c->scratch_doubles >= doubles) return CHORUS_OK;
+    cudaFree(c->d_scratch);
+    c->d_scratch = nullptr;
+    c->scratch_doubles = 0;
+    CU(c, cudaMalloc(&c->d_scratch, sizeof(double) * doubles));
+    c->scratch_doubles = doubles;
+    return CHORUS_OK;
+  }
+  template <bool DIFF, int GRADV, bool SPILL>
+  static int residual_launch_impl(chorus_ctx* c, const double* Qin, const StageOut& out) {
+    constexpr size_t smem = residual_smem_bytes<N, DIFF, GRADV, SPILL>();
     if (smem > c->max_smem)
       return fail(c, CHORUS_EINVAL, "order " + std::to_string(N) + " with these physics flags needs " + std::to_string(smem) +
                                         " B of shared memory per CTA (limit " + std::to_string(c->max_smem) + ")");
-    auto k = residual_kernel<N, DIFF, GRADV>;
+    auto k = residual_kernel<N, DIFF, GRADV, SPILL>;
     CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 1;
     CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, smem));
     if (occ < 1) occ = 1;
     const int64_t cap = (int64_t)c->num_sms * occ;
     const int grid = (int)(c->E < cap ? c->E : cap);
+    if (SPILL) {
+      int rc = need_scratch(c, residual_scratch_doubles<N, DIFF, GRADV>() * (size_t)grid);
+      if (rc) return rc;
+    }
     {
       ProfScope ps(c, 2);
       k<<<grid, 256, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf[0], c->d_Vf, c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl,
-                                         c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient, out);
+                                         c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient, out, c->d_scratch);
     }
     ++c->launches;
     CU(c, cudaGetLastError());
     return CHORUS_OK;
+  }
+  template <bool DIFF, int GRADV>
+  static int residual_launch(chorus_ctx* c, const double* Qin, const StageOut& out) {
+    if (residual_smem_bytes<N, DIFF, GRADV, false>() <= c->max_smem) return residual_launch_impl<DIFF, GRADV, false>(c, Qin, out);
+    return residual_launch_impl<DIFF, GRADV, true>(c, Qin, out);
   }
   // ---- production pipeline (orders 4..7): main kernel, then (diffusion) the face kernel
   template <bool DIFF, int GRADV>
@@ -205,24 +226,33 @@ struct Hot {
     CU(c, cudaGetLastError());
     return CHORUS_OK;
   }
-  static int grad(chorus_ctx* c, const double* Qin, double* Vf, double* Gout) {
-    constexpr size_t smem = grad_smem_bytes<N>();
+  template <bool SPILL>
+  static int grad_impl(chorus_ctx* c, const double* Qin, double* Vf, double* Gout) {
+    constexpr size_t smem = grad_smem_bytes<N, SPILL>();
     if (smem > c->max_smem) return fail(c, CHORUS_EINVAL, "gradient kernel: order too high for the shared-memory budget");
-    auto k = grad_kernel<N>;
+    auto k = grad_kernel<N, SPILL>;
     CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 1;
     CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, smem));
     if (occ < 1) occ = 1;
     const int64_t cap = (int64_t)c->num_sms * occ;
     const int grid = (int)(c->E < cap ? c->E : cap);
+    if (SPILL) {
+      int rc = need_scratch(c, (size_t)27 * I::n3 * (size_t)grid);
+      if (rc) return rc;
+    }
     {
       ProfScope ps(c, 1);
       k<<<grid, 256, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf[0], c->d_Sfl, c->d_jinv, c->d_krfl, c->d_nbr_elem, c->d_nbr_face,
-                                         c->d_nbr_orient, Vf, Gout);
+                                         c->d_nbr_orient, Vf, Gout, c->d_scratch);
     }
     ++c->launches;
     CU(c, cudaGetLastError());
     return CHORUS_OK;
+  }
+  static int grad(chorus_ctx* c, const double* Qin, double* Vf, double* Gout) {
+    if (grad_smem_bytes<N, false>() <= c->max_smem) return grad_impl<false>(c, Qin, Vf, Gout);
+    return grad_impl<true>(c, Qin, Vf, Gout);
   }
   // legacy three-kernel path (orders 2, 3, 8, 9 and CHORUS_KERNELS=scalar): trace, gradient, residual + RK
   static int stage_legacy(chorus_ctx* c, const double* Qin, const StageOut& out) {
@@ -399,7 +429,7 @@ void chorus_free(chorus_ctx* c) {
   cudaFree(c->d_Gm); cudaFree(c->d_Dff); cudaFree(c->d_Efs); cudaFree(c->d_Dfs);
   cudaFree(c->d_Sfl); cudaFree(c->d_detJ); cudaFree(c->d_jinv); cudaFree(c->d_xsol); cudaFree(c->d_krfl); cudaFree(c->d_nfc);
   for (int k = 0; k < 5; ++k) cudaFree(c->d_U[k]);
-  cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_ws); cudaFree(c->d_arrivals);
+  cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_ws); cudaFree(c->d_arrivals); cudaFree(c->d_scratch);
   for (auto& v : c->prof_ev)
     for (auto& ev : v) {
       cudaEventDestroy(ev.first);

@@ -89,17 +89,18 @@ __device__ __forceinline__ void br1_gradient(const ElemNbr& nb, const double* sQ
 // On wall faces the final wall viscous flux (stress-free, thermal and magnetic wall options) is stored instead.
 // Optionally writes the gradient itself (test accessor chorus_get_gradient): Gout [E][27][n3].
 // ---------------------------------------------------------------------------------------------------------
-template <int N>
+// SPILL: the gradient lives in a per-CTA scratch area in global memory (n = 9: 36 n^3 doubles do not fit in shared memory)
+template <int N, bool SPILL = false>
 __global__ void __launch_bounds__(256) grad_kernel(int64_t E, PhysD ph, const double* __restrict__ Qe, const double* __restrict__ Qf,
                                                    const double* __restrict__ Sfl, const double* __restrict__ jinv,
                                                    const double* __restrict__ krfl, const int32_t* __restrict__ nbr_elem,
                                                    const uint8_t* __restrict__ nbr_face, const uint8_t* __restrict__ nbr_orient,
-                                                   double* __restrict__ Vf, double* __restrict__ Gout) {
+                                                   double* __restrict__ Vf, double* __restrict__ Gout, double* scratch) {
   using I = Ix<N>;
   extern __shared__ double sm[];
   double* sQ = sm;                       // [9][n3]
-  double* sG = sQ + 9 * I::n3;           // [27][n3]
-  double* sQo = sG + 27 * I::n3;         // [6][9][n2]
+  double* sG = SPILL ? scratch + blockIdx.x * (size_t)27 * I::n3 : sQ + 9 * I::n3;   // [27][n3]
+  double* sQo = sQ + (SPILL ? 9 : 36) * I::n3;                                        // [6][9][n2]
   double* sQn = sQo + 54 * I::n2;        // [6][9][n2]
   __shared__ ElemNbr nb;
   const OpsC& op = c_ops[N];

@@ -18,12 +18,14 @@ struct StageOut {
 };
 
 // GRADV: 0 no gradient needed, 1 gradient of B only (Powell sources without diffusion), 2 all nine variables.
-template <int N, bool DIFF, int GRADV>
+// SPILL: orders whose tiles exceed the shared memory of an SM (n = 8, 9 with diffusion) keep the neighbour traces, the gradient
+// and its interpolant in a per-CTA scratch area in global memory (L2-resident: the grid is persistent) instead.
+template <int N, bool DIFF, int GRADV, bool SPILL = false>
 __global__ void __launch_bounds__(256, 1)
 residual_kernel(int64_t E, PhysD ph, const double* __restrict__ Qe, const double* __restrict__ Qf, const double* __restrict__ Vf,
                 const double* __restrict__ Sfl, const double* __restrict__ detJ, const double* __restrict__ jinv,
                 const double* __restrict__ xsol, const double* __restrict__ krfl, const int32_t* __restrict__ nbr_elem,
-                const uint8_t* __restrict__ nbr_face, const uint8_t* __restrict__ nbr_orient, StageOut out) {
+                const uint8_t* __restrict__ nbr_face, const uint8_t* __restrict__ nbr_orient, StageOut out, double* scratch) {
   using I = Ix<N>;
   static_assert(!DIFF || GRADV == 2, "diffusion needs the gradient of all variables");
   constexpr int NGV = GRADV == 2 ? 9 : GRADV == 1 ? 3 : 0;
@@ -33,7 +35,8 @@ residual_kernel(int64_t E, PhysD ph, const double* __restrict__ Qe, const double
   double* sR = sQ + 9 * I::n3;                    // [9][n3]        xi-divergence accumulator
   double* sH = sR + 9 * I::n3;                    // [9][N+1][n2]   Q^ then F~ of the current family, line-major
   double* sQo = sH + 9 * I::nf;                   // [6][9][n2]
-  double* sQn = sQo + 54 * I::n2;                 // [6][9][n2]
+  constexpr size_t kScratch = (size_t)54 * I::n2 + 3 * NGV * I::n3 + (DIFF ? 27 * (N - 1) * I::n2 : 0);
+  double* sQn = SPILL ? scratch + blockIdx.x * kScratch : sQo + 54 * I::n2;      // [6][9][n2]
   double* sG = sQn + 54 * I::n2;                  // [3*NGV][n3]
   double* sGh = sG + 3 * NGV * I::n3;             // [27][N-1][n2]  (DIFF only)
   __shared__ ElemNbr nb;
@@ -200,15 +203,20 @@ residual_kernel(int64_t E, PhysD ph, const double* __restrict__ Qe, const double
 }
 
 template <int N, bool DIFF, int GRADV>
-constexpr size_t residual_smem_bytes() {
+constexpr size_t residual_scratch_doubles() {     // per CTA, SPILL only
   using I = Ix<N>;
   constexpr int NGV = GRADV == 2 ? 9 : GRADV == 1 ? 3 : 0;
-  return sizeof(double) * (size_t)(18 * I::n3 + 9 * I::nf + 108 * I::n2 + 3 * NGV * I::n3 + (DIFF ? 27 * (N - 1) * I::n2 : 0));
+  return (size_t)54 * I::n2 + 3 * NGV * I::n3 + (DIFF ? 27 * (N - 1) * I::n2 : 0);
 }
-template <int N>
+template <int N, bool DIFF, int GRADV, bool SPILL = false>
+constexpr size_t residual_smem_bytes() {
+  using I = Ix<N>;
+  return sizeof(double) * ((size_t)(18 * I::n3 + 9 * I::nf + 54 * I::n2) + (SPILL ? 0 : residual_scratch_doubles<N, DIFF, GRADV>()));
+}
+template <int N, bool SPILL = false>
 constexpr size_t grad_smem_bytes() {
   using I = Ix<N>;
-  return sizeof(double) * (size_t)(36 * I::n3 + 108 * I::n2);
+  return sizeof(double) * (size_t)((SPILL ? 9 : 36) * I::n3 + 108 * I::n2);
 }
 
 }  // namespace chorus

@@ -391,10 +391,9 @@ def workload(name: str) -> Workload:
         "sweep_n5": Workload("sweep_n5", 5, 34, 12, 3.0, 4, 1e-3, True, 2, sh3),
         "sweep_n6": Workload("sweep_n6", 6, 28, 10, 3.0, 4, 1e-3, True, 2, sh3),
         "sweep_n7": Workload("sweep_n7", 7, 24, 8, 3.0, 4, 1e-3, True, 2, sh3),
-        # orders 8 and 9 run on the scalar path, whose diffusive element kernel does not fit in shared memory: diffusion off,
-        # which is what BASELINE.json's configs[4] asks for ("seeded perturbations as in config 0")
-        "sweep_n8": Workload("sweep_n8", 8, 22, 7, 3.0, 4, 0.0, True, 2, sh3),
-        "sweep_n9": Workload("sweep_n9", 9, 18, 7, 3.0, 4, 0.0, True, 2, sh3),
+        # orders 8 and 9 run on the scalar three-kernel path (with diffusion its gradient tiles live in a global scratch area)
+        "sweep_n8": Workload("sweep_n8", 8, 22, 7, 3.0, 4, 1e-3, True, 2, sh3),
+        "sweep_n9": Workload("sweep_n9", 9, 18, 7, 3.0, 4, 1e-3, True, 2, sh3),
     }
     return table[name]
 

@@ -142,7 +142,8 @@ def test_all_orientation_codes_parity():
         assert np.abs(g.residual()).max() <= 1e-13 * a.max()
 
 
-@pytest.mark.parametrize("n,diff", [(2, 1e-3), (3, 1e-3), (4, 1e-3), (5, 1e-3), (6, 1e-3), (7, 0.0), (8, 0.0)])
+@pytest.mark.parametrize("n,diff", [(2, 1e-3), (3, 1e-3), (4, 1e-3), (5, 1e-3), (6, 1e-3), (7, 0.0), (7, 1e-3), (8, 0.0),
+                                    (8, 1e-3), (9, 0.0), (9, 1e-3)])
 def test_order_sweep_parity(n, diff):
     """BASELINE config 4 (order sweep), at sizes the oracle finishes in seconds."""
     w, mesh, o, g, Q, phys = shell_case(n, 3, 2, 3.0, 4, diff)

@@ -271,7 +271,12 @@ template <int R>
 __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(R)); }
 
 constexpr int kMainThreads = 256;     // warpgroup 0: chain warps (DMMA), warpgroup 1: helper warps (memory, faces, sources, RK)
-constexpr int kChainRegs = 160, kHelpRegs = 96;   // 128 * (160 + 96) = the CTA's 256 * 128 registers: two CTAs per SM
+// 128 * (chain + helper) = the CTA's 256 * 128 registers: two CTAs per SM.  With diffusion the chain warps carry the streamed
+// viscous flux state and need 160; without it they are light and the helpers (sources, RK, next-state traces) get the room.
+#ifndef CHORUS_NODIFF_CHAIN_REGS
+#define CHORUS_NODIFF_CHAIN_REGS 144
+#endif
+template <bool DIFF> struct RegSplit { static constexpr int kChain = DIFF ? 160 : CHORUS_NODIFF_CHAIN_REGS, kHelp = 256 - kChain; };
 
 // per-thread constants of the DMMA mapping
 template <int N>
@@ -582,7 +587,8 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
 
   if (wg == 0) {
     // =============================================== chain warps ===============================================
-    setmaxnreg_inc<kChainRegs>();
+    if (RegSplit<DIFF>::kChain > 128) setmaxnreg_inc<RegSplit<DIFF>::kChain>();
+    else if (RegSplit<DIFF>::kChain < 128) setmaxnreg_dec<RegSplit<DIFF>::kChain>();
     const OpsC& op = c_ops[N];
     const int lane = tid & 31, warp = tid >> 5;
     const bool active = warp < M::kWarps;
@@ -726,7 +732,8 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     }
   } else {
     // =============================================== helper warps ==============================================
-    setmaxnreg_dec<kHelpRegs>();
+    if (RegSplit<DIFF>::kHelp < 128) setmaxnreg_dec<RegSplit<DIFF>::kHelp>();
+    else if (RegSplit<DIFF>::kHelp > 128) setmaxnreg_inc<RegSplit<DIFF>::kHelp>();
     constexpr int P2 = (I::n3 + H - 1) / H;              // solution points per helper thread
     // connectivity of the element this CTA handles next, fetched one element ahead by helper threads 0..5
     int pn_e = 0, pn_f = 0, pn_o = 0;

@@ -45,6 +45,12 @@ struct Mma {
   static constexpr int kTPD = (FG + kWarps - 1) / kWarps;     // directional tasks per warp and direction
   static constexpr int kTail = (3 * LO + 7) / 8;               // tail tasks per element
   static_assert(kTail <= kWarps, "tail tasks: one round");
+  // Small orders (n <= 5): an element's tiles leave room for one divergence accumulator PER DIRECTION, so no two tasks ever
+  // touch the same word: all 3 FG + kTail tasks of an element are dealt to the four chain warps with no barrier in between
+  // (n = 4: 6 tasks, n = 5: 10) instead of FG tasks per barrier-separated direction round.
+  static constexpr bool kFree = N <= 5;
+  static constexpr int kTasks = 3 * FG + kTail;              // kFree: tasks per element ...
+  static constexpr int kTPW = (kTasks + 3) / 4;               // ... and per chain warp
   // left-over lines (a,b): d = 0: b = 0, a < LO;  d = 1: b = 1, a < LO;  d = 2: a, b >= LO, the first LO of them
   __host__ __device__ static constexpr bool is_lo(int d, int ab) {
     const int a = ab % N, b = ab / N;
@@ -348,7 +354,8 @@ __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, c
 // WAITF: this is the element's first chain task of the warp: the common face fluxes (written by the helper warps beside the
 // chain rule and the first interpolations) are awaited here, just before they are needed, and the left-over direction-0
 // points of sR are zeroed.
-template <int N, bool DIFF, int D, bool WAITF = false>
+// STORE: 1 store the divergence contribution, 0 accumulate it, -1 (default): store for direction 0, accumulate otherwise.
+template <int N, bool DIFF, int D, bool WAITF = false, int STORE = -1>
 __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, const ElemNbr& nb, const StageIO& io, const Geo& geo,
                                           int64_t e, const double* sQ, const double* sG, const double* sFace, const double* sS, double* sR,
                                           int ln, bool lv, int dd = 0, int ctid = 0) {
@@ -456,7 +463,7 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
     // Direction 0 stores into sR, the others accumulate; the points of the left-over direction-0 lines, which no direction-0
     // task touches, start from zero (they are first accumulated into after the next chain-warp barrier).
     using MM = Mma<N>;
-    if constexpr (MM::LO > 0) {
+    if constexpr (MM::LO > 0 && !MM::kFree) {
       for (int t = ctid; t < 9 * MM::LO * N; t += 32 * MM::kWarps) {
         const int l = t % N, i = (t / N) % MM::LO, v = t / (N * MM::LO);
         sR[v * I::n3 + I::sbase(0, MM::line_of(0, 8 * MM::FG + i)) + l] = 0.0;
@@ -502,8 +509,9 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
   for (int v = 0; v < 9; ++v) dmma884(r0[v], r1[v], q1[v], L.bD1);
 #pragma unroll
   for (int v = 0; v < 9; ++v) {
-    if (ok0) out[v * I::n3] = (D == 0) ? r0[v] : out[v * I::n3] + r0[v];
-    if (ok1) out[v * I::n3 + st] = (D == 0) ? r1[v] : out[v * I::n3 + st] + r1[v];
+    constexpr bool kStore = STORE == 1 || (STORE == -1 && D == 0);
+    if (ok0) out[v * I::n3] = kStore ? r0[v] : out[v * I::n3] + r0[v];
+    if (ok1) out[v * I::n3 + st] = kStore ? r1[v] : out[v * I::n3 + st] + r1[v];
   }
 }
 
@@ -568,6 +576,8 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   double* sS = sQn + ev(54 * I::n2);     // [3 fam][3 comp][nf] S^d at the flux points (cp.async; 9*nf is even)
   double* sG = sS + 9 * I::nf;           // [3*NGV][n3]
   double* sR = sQo;
+  double* sR12 = sG + ev(3 * NGV * I::n3);   // kFree: the accumulators of directions 1 and 2, [2][9][n3] (direction 0: sR)
+  constexpr int kRS = ev(9 * I::n3);
   __shared__ ElemNbr nb;
   __shared__ int s_second;
   __shared__ __align__(8) uint64_t mbar;   // completion of the bulk (TMA) copies of one element
@@ -633,6 +643,27 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         const int g = warp + k * M::kWarps;
         lnd[d][k] = M::line_of(d, (g < M::FG ? g : 0) * 8 + L.r);
       }
+    // kFree: task i = warp + 4 t of this warp: direction, line of this thread's row, validity of the row
+    int fd[M::kTPW], fl[M::kTPW];
+    bool fv[M::kTPW], fr[M::kTPW];        // task exists / row carries a line
+#pragma unroll
+    for (int t = 0; t < M::kTPW; ++t) {
+      const int i = warp + 4 * t;
+      fv[t] = M::kFree && i < M::kTasks;
+      fr[t] = fv[t];
+      fd[t] = 0; fl[t] = 0;
+      if (fv[t]) {
+        if (i < 3 * M::FG) {
+          fd[t] = i / M::FG;
+          fl[t] = M::line_of(fd[t], (i % M::FG) * 8 + L.r);
+        } else {
+          const int q = (i - 3 * M::FG) * 8 + L.r;            // index among the 3 LO left-over lines
+          fr[t] = q < 3 * M::LO;
+          fd[t] = fr[t] ? q / (M::LO > 0 ? M::LO : 1) : 0;
+          fl[t] = M::line_of(fd[t], 8 * M::FG + (fr[t] ? q % (M::LO > 0 ? M::LO : 1) : 0));
+        }
+      }
+    }
     // tail tasks rotate over the warps (hence over the SM sub-partitions) from element to element, and every second CTA
     // arriving on an SM starts half a turn ahead
     int tail_rot = s_second ? M::kWarps / 2 : 0;
@@ -669,7 +700,11 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       bar_sync(kBarIn, kMainThreads);          // inputs and wall states are in shared memory
       CHORUS_TICK(1);
       // ---- A3: BR1 gradient.  d/dxi_d by DMMA, then the chain rule per point.
-      if constexpr (GRADV != 0) {
+      if constexpr (GRADV != 0 && M::kFree) {
+#pragma unroll
+        for (int t = 0; t < M::kTPW; ++t)
+          if (fv[t]) grad_dir<N, NGV, GV0, 3>(L, nb, sQ, sQo, sQn, sG, fl[t], fr[t], fd[t]);
+      } else if constexpr (GRADV != 0) {
         if (active) {
 #pragma unroll
           for (int k = 0; k < M::kTPD; ++k)
@@ -699,33 +734,44 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       }
       bar_sync(kBarChain, H);                  // the gradient is complete in shared memory
       CHORUS_TICK(3);
-      // ---- A1, A4, A5, A7: one DMMA chain per warp and direction, directions separated by chain-warp barriers
-      if (active) {
-        chain_dir<N, DIFF, 0, true>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[0][0], true, 0, tid);
+      if constexpr (M::kFree) {
+        // ---- A1, A4, A5, A7: every task stores into the accumulator of its own direction; no barrier between tasks
 #pragma unroll
-        for (int k = 1; k < M::kTPD; ++k)
-          if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 0>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[0][k], true);
+        for (int t = 0; t < M::kTPW; ++t) {
+          if (!fv[t]) continue;
+          double* acc = fd[t] == 0 ? sR : sR12 + (fd[t] - 1) * kRS;
+          if (t == 0) chain_dir<N, DIFF, 3, true, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, acc, fl[t], fr[t], fd[t], tid);
+          else chain_dir<N, DIFF, 3, false, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, acc, fl[t], fr[t], fd[t]);
+        }
       } else {
-        bar_sync(kBarFaces, kMainThreads);
-      }
-      bar_sync(kBarChain, H);
-      CHORUS_TICK(4);
-      if (active) {
+      // ---- A1, A4, A5, A7: one DMMA chain per warp and direction, directions separated by chain-warp barriers
+        if (active) {
+          chain_dir<N, DIFF, 0, true>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[0][0], true, 0, tid);
 #pragma unroll
-        for (int k = 0; k < M::kTPD; ++k)
-          if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
-      }
-      bar_sync(kBarChain, H);
-      CHORUS_TICK(5);
-      if (active) {
-#pragma unroll
-        for (int k = 0; k < M::kTPD; ++k)
-          if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
-      }
-      if (M::kTail > 0) {   // left-over lines of the three directions: no two of them share a solution point
+          for (int k = 1; k < M::kTPD; ++k)
+            if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 0>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[0][k], true);
+        } else {
+          bar_sync(kBarFaces, kMainThreads);
+        }
         bar_sync(kBarChain, H);
-        CHORUS_TICK(6);
-        if (active && tw < M::kTail) chain_dir<N, DIFF, 3>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, tl_ln, tl_ok, tl_d);
+        CHORUS_TICK(4);
+        if (active) {
+#pragma unroll
+          for (int k = 0; k < M::kTPD; ++k)
+            if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
+        }
+        bar_sync(kBarChain, H);
+        CHORUS_TICK(5);
+        if (active) {
+#pragma unroll
+          for (int k = 0; k < M::kTPD; ++k)
+            if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
+        }
+        if (M::kTail > 0) {   // left-over lines of the three directions: no two of them share a solution point
+          bar_sync(kBarChain, H);
+          CHORUS_TICK(6);
+          if (active && tw < M::kTail) chain_dir<N, DIFF, 3>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, tl_ln, tl_ok, tl_d);
+        }
       }
       bar_sync(kBarRes, kMainThreads);         // divergence accumulated: the helpers finish the element
       CHORUS_TICK(7);
@@ -912,7 +958,11 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         if (s < I::n3) {
           double R[9];
 #pragma unroll
-          for (int v = 0; v < 9; ++v) R[v] = w[q] * sR[v * I::n3 + s] + K[q][v];
+          for (int v = 0; v < 9; ++v) {
+            double dv = sR[v * I::n3 + s];
+            if (M::kFree) dv += sR12[v * I::n3 + s] + sR12[kRS + v * I::n3 + s];     // one accumulator per direction
+            R[v] = w[q] * dv + K[q][v];
+          }
           if (DIFF) {                    // finished by the face kernel
 #pragma unroll
             for (int v = 0; v < 9; ++v) io.Part[(e * 9 + v) * I::n3 + s] = R[v];
@@ -948,7 +998,8 @@ constexpr size_t stage_main_smem_bytes() {
   constexpr int NGV = GRADV == 2 ? 9 : GRADV == 1 ? 3 : 0;
   constexpr int kOwn = 54 * I::n2 > 9 * I::n3 ? 54 * I::n2 : 9 * I::n3;
   constexpr auto ev = [](int x) { return (x + 1) & ~1; };
-  return sizeof(double) * (size_t)(ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + 9 * I::nf + 3 * NGV * I::n3);
+  return sizeof(double) * (size_t)(ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + 9 * I::nf + ev(3 * NGV * I::n3) +
+                                   (Mma<N>::kFree ? 2 * ev(9 * I::n3) : 0));
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -30,6 +30,21 @@ NSTAGES = 5
 # "diffusion on": HBM bytes (whole stage, element kernel's share) and flop (whole stage, element kernel's share).
 ALG_BYTES = {True: (660.0, 532.0), False: (548.0, 548.0)}
 ALG_FLOPS = {True: (3550.0, 3360.0), False: (1370.0, 1370.0)}
+# Other orders, full physics: n -> (flop, bytes) per point per stage, whole stage.
+ALG_BY_ORDER = {4: (3008.0, 794.0), 5: (3267.0, 714.0), 6: (3550.0, 660.0), 7: (3840.0, 622.0), 8: (4141.0, 593.0), 9: (4447.0, 571.0)}
+
+
+def alg_work(n, diff):
+    """((stage_bytes, kernel_bytes), (stage_flops, kernel_flops)) per solution point per stage for order n.
+    The element kernel's share of the stage is scaled from the n = 6 split (the rest is the viscous face kernel: face
+    correction and next traces); without diffusion only the n = 6 figures exist and are scaled by the full-physics ratio."""
+    if n == 6:
+        return ALG_BYTES[diff], ALG_FLOPS[diff]
+    f, b = ALG_BY_ORDER.get(n, ALG_BY_ORDER[6])
+    if not diff:
+        f, b = f * 1370.0 / 3550.0, b * 548.0 / 660.0
+        return (b, b), (f, f)
+    return (b, b * 532.0 / 660.0), (f, f * 3360.0 / 3550.0)
 FP64_PEAK_TFLOPS = 37.2   # 148 SMs x 4 sub-partitions x 16 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7.3; DMMA measured 37.0)
 
 
@@ -260,8 +275,7 @@ def main():
     hbm_peak, peak_src = measured_peaks()
     main_ms, main_cnt = prof["main"]
     main_avg_ms = main_ms / max(main_cnt, 1)
-    stage_bytes, kernel_bytes = ALG_BYTES[diff]
-    stage_flops, kernel_flops = ALG_FLOPS[diff]
+    (stage_bytes, kernel_bytes), (stage_flops, kernel_flops) = alg_work(n, diff)
     achieved = kernel_flops * pts / (main_avg_ms * 1e-3) / 1e12 if main_cnt else None        # TFLOP/s of the element kernel
     kernel_ms = {k: (v[0] / max(v[1], 1)) for k, v in prof.items()}
     stage_ms = ms / (args.steps * NSTAGES)
@@ -273,7 +287,7 @@ def main():
                             solution_points=pts, N_rho=w.N_rho, diffusion=w.diffusion, rk="SSPRK(5,3)",
                             parallelism="replicas" if world > 1 else "single GPU", l2="inputs larger than L2 (state %.0f MB)" % (pts * 72 / 1e6)),
                 clocks=clocks.summary(), gpu_launches=launches,
-                roofline=dict(bound="alu", kernel="stage_main_kernel", achieved=achieved, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
+                roofline=dict(bound="alu", kernel="stage_main_kernel" if 4 <= n <= 7 else "residual_kernel", achieved=achieved, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
                               frac=(achieved / FP64_PEAK_TFLOPS) if achieved else None, traffic=ncu_traffic(args.workload),
                               peak_source="nominal FP64 pipe: 148 SMs x 4 x 16 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7.3)",
                               measured_fp64=peaks, alg_flops_per_point=kernel_flops, alg_bytes_per_point=kernel_bytes,

@@ -151,7 +151,7 @@ struct Hot {
   static int main_launch(chorus_ctx* c, const StageIO& io) {
     if constexpr (N >= 4 && N <= 7) {
       constexpr size_t smem = stage_main_smem_bytes<N, GRADV>();
-      constexpr int threads = kMainThreads;
+      constexpr int threads = MainCfg<N>::kThreads;
       auto k = stage_main_kernel<N, DIFF, GRADV>;
       CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       CU(c, cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));

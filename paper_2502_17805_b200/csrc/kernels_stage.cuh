@@ -41,7 +41,9 @@ struct Mma {
   // their own direction at run time.  At most 4 warps per CTA: warp w runs on SM sub-partition w % 4, so a fifth warp
   // would double the load of one FP64 pipe (measured: 5 warps of DMMA take twice as long as 4).
   static constexpr int FG = I::n2 / 8, LO = I::n2 % 8;
-  static constexpr int kWarps = FG < 4 ? FG : 4;
+  // n = 7 leaves room for only one CTA per SM (173 KB of tiles): it gets two chain warpgroups, two chain warps per sub-partition
+  static constexpr int kChainWG = N == 7 ? 2 : 1;
+  static constexpr int kWarps = FG < 4 * kChainWG ? FG : 4 * kChainWG;
   static constexpr int kTPD = (FG + kWarps - 1) / kWarps;     // directional tasks per warp and direction
   static constexpr int kTail = (3 * LO + 7) / 8;               // tail tasks per element
   static_assert(kTail <= kWarps, "tail tasks: one round");
@@ -276,13 +278,23 @@ __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.
 template <int R>
 __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(R)); }
 
-constexpr int kMainThreads = 256;     // warpgroup 0: chain warps (DMMA), warpgroup 1: helper warps (memory, faces, sources, RK)
+// thread layout of the element kernel: chain warpgroup(s) first (DMMA), then one helper warpgroup (memory, faces, sources, RK)
+template <int N> struct MainCfg {
+  static constexpr int kChainWG = N == 7 ? 2 : 1;
+  static constexpr int kThreads = 128 * (kChainWG + 1);
+  static constexpr int kMinBlocks = kChainWG == 2 ? 1 : 2;
+};
 // 128 * (chain + helper) = the CTA's 256 * 128 registers: two CTAs per SM.  With diffusion the chain warps carry the streamed
 // viscous flux state and need 160; without it they are light and the helpers (sources, RK, next-state traces) get the room.
 #ifndef CHORUS_NODIFF_CHAIN_REGS
 #define CHORUS_NODIFF_CHAIN_REGS 144
 #endif
-template <bool DIFF> struct RegSplit { static constexpr int kChain = DIFF ? 160 : CHORUS_NODIFF_CHAIN_REGS, kHelp = 256 - kChain; };
+template <bool DIFF, int CWG = 1> struct RegSplit {
+  // one chain warpgroup: launch at 128 registers (two CTAs per SM); two: launch at 168 (one CTA), 2 x 200 + 96 <= 3 x 168
+  static constexpr int kLaunch = CWG == 2 ? 168 : 128;
+  static constexpr int kChain = CWG == 2 ? 200 : DIFF ? 160 : CHORUS_NODIFF_CHAIN_REGS;
+  static constexpr int kHelp = CWG == 2 ? 96 : 256 - kChain;
+};
 
 // per-thread constants of the DMMA mapping
 template <int N>
@@ -459,7 +471,7 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
     }
   }
   if (WAITF) {
-    bar_sync(kBarFaces, kMainThreads);     // common face fluxes are in sFace; own traces are dead: their region becomes sR
+    bar_sync(kBarFaces, MainCfg<N>::kThreads);     // common face fluxes are in sFace; own traces are dead: their region becomes sR
     // Direction 0 stores into sR, the others accumulate; the points of the left-over direction-0 lines, which no direction-0
     // task touches, start from zero (they are first accumulated into after the next chain-warp barrier).
     using MM = Mma<N>;
@@ -560,7 +572,7 @@ __device__ unsigned long long g_phase_cycles[16];
 // Barriers per element: IN (inputs ready) -> GRAD (gradient DMMAs done, face fluxes in registers) -> CHAINRULE (gradient and
 // face fluxes in shared memory) -> RES (divergence accumulated).
 template <int N, bool DIFF, int GRADV>
-__global__ void __launch_bounds__(kMainThreads, 2)
+__global__ void __launch_bounds__(MainCfg<N>::kThreads, MainCfg<N>::kMinBlocks)
 stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   using I = Ix<N>;
   using M = Mma<N>;
@@ -589,16 +601,20 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   __syncthreads();
-  const int wg = threadIdx.x >> 7, tid = threadIdx.x & 127;
+  constexpr int kMainThreads = MainCfg<N>::kThreads, kCT = 128 * M::kChainWG;      // all threads / chain threads
+  using RS = RegSplit<DIFF, M::kChainWG>;
+  const bool is_chain = M::kChainWG == 1 ? (threadIdx.x >> 7) == 0 : threadIdx.x < kCT;
+  const int tid = M::kChainWG == 1 ? (int)(threadIdx.x & 127) : is_chain ? (int)threadIdx.x : (int)threadIdx.x - kCT;
   // The contiguous per-element blocks (state, own traces, S^d) go by TMA bulk copy when they are 16-byte aligned (n even);
   // the neighbour traces are gathered through the orientation map with 8-byte cp.async either way.
   constexpr bool kBulk = (9 * I::n3) % 2 == 0 && (54 * I::n2) % 2 == 0;
-  constexpr int H = 128;                 // threads per warpgroup
+  constexpr int H = 128;                 // helper threads
 
-  if (wg == 0) {
+  if (is_chain) {
     // =============================================== chain warps ===============================================
-    if (RegSplit<DIFF>::kChain > 128) setmaxnreg_inc<RegSplit<DIFF>::kChain>();
-    else if (RegSplit<DIFF>::kChain < 128) setmaxnreg_dec<RegSplit<DIFF>::kChain>();
+    constexpr int CH = kCT;              // chain threads
+    if (RS::kChain > RS::kLaunch) setmaxnreg_inc<RS::kChain>();
+    else if (RS::kChain < RS::kLaunch) setmaxnreg_dec<RS::kChain>();
     const OpsC& op = c_ops[N];
     const int lane = tid & 31, warp = tid >> 5;
     const bool active = warp < M::kWarps;
@@ -667,7 +683,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     // tail tasks rotate over the warps (hence over the SM sub-partitions) from element to element, and every second CTA
     // arriving on an SM starts half a turn ahead
     int tail_rot = s_second ? M::kWarps / 2 : 0;
-    constexpr int P2 = (I::n3 + H - 1) / H;     // solution points per chain thread in the chain rule
+    constexpr int P2 = (I::n3 + CH - 1) / CH;     // solution points per chain thread in the chain rule
 #ifdef CHORUS_PHASE_TIMING
     long long tick_ = clock64();
 #endif
@@ -689,7 +705,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       if (GRADV != 0) {
 #pragma unroll
         for (int q = 0; q < P2; ++q) {
-          const int s = tid + q * H;
+          const int s = tid + q * CH;
           const int sc = s < I::n3 ? s : 0;
 #pragma unroll
           for (int k = 0; k < 9; ++k) jv[q][k] = geo.jinv[e * 9 * I::n3 + k * I::n3 + sc];
@@ -721,7 +737,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       if constexpr (GRADV != 0) {
 #pragma unroll
         for (int q = 0; q < P2; ++q) {
-          const int s = tid + q * H;
+          const int s = tid + q * CH;
           if (s < I::n3) {
 #pragma unroll
             for (int vv = 0; vv < NGV; ++vv) {
@@ -732,7 +748,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           }
         }
       }
-      bar_sync(kBarChain, H);                  // the gradient is complete in shared memory
+      bar_sync(kBarChain, CH);                  // the gradient is complete in shared memory
       CHORUS_TICK(3);
       if constexpr (M::kFree) {
         // ---- A1, A4, A5, A7: every task stores into the accumulator of its own direction; no barrier between tasks
@@ -753,14 +769,14 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         } else {
           bar_sync(kBarFaces, kMainThreads);
         }
-        bar_sync(kBarChain, H);
+        bar_sync(kBarChain, CH);
         CHORUS_TICK(4);
         if (active) {
 #pragma unroll
           for (int k = 0; k < M::kTPD; ++k)
             if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
         }
-        bar_sync(kBarChain, H);
+        bar_sync(kBarChain, CH);
         CHORUS_TICK(5);
         if (active) {
 #pragma unroll
@@ -768,7 +784,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
             if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
         }
         if (M::kTail > 0) {   // left-over lines of the three directions: no two of them share a solution point
-          bar_sync(kBarChain, H);
+          bar_sync(kBarChain, CH);
           CHORUS_TICK(6);
           if (active && tw < M::kTail) chain_dir<N, DIFF, 3>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, tl_ln, tl_ok, tl_d);
         }
@@ -778,8 +794,8 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     }
   } else {
     // =============================================== helper warps ==============================================
-    if (RegSplit<DIFF>::kHelp < 128) setmaxnreg_dec<RegSplit<DIFF>::kHelp>();
-    else if (RegSplit<DIFF>::kHelp > 128) setmaxnreg_inc<RegSplit<DIFF>::kHelp>();
+    if (RS::kHelp < RS::kLaunch) setmaxnreg_dec<RS::kHelp>();
+    else if (RS::kHelp > RS::kLaunch) setmaxnreg_inc<RS::kHelp>();
     constexpr int P2 = (I::n3 + H - 1) / H;              // solution points per helper thread
     // connectivity of the element this CTA handles next, fetched one element ahead by helper threads 0..5
     int pn_e = 0, pn_f = 0, pn_o = 0;

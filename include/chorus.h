@@ -19,8 +19,9 @@
  *   order) maps an own face point (a,b) to the coinciding neighbour face point (a',b').
  *
  * Ownership: the caller owns every buffer it passes.  chorus_init copies the mesh; the library owns all
- * device arrays until chorus_free.  One opaque context per mesh; no global state; contexts are not
- * thread-safe.  All work is enqueued on the cudaStream_t given to chorus_init; calls that take or return
+ * device arrays until chorus_free.  One opaque context per mesh; contexts are not thread-safe.  The only
+ * process-wide state is the table of 1-D operators in __constant__ memory, indexed by the order: chorus_init writes
+ * the entry of its order with values that depend on the order alone, so contexts of any orders coexist.  All work is enqueued on the cudaStream_t given to chorus_init; calls that take or return
  * HOST data synchronise that stream, calls with on_device = 1 are asynchronous on it.
  *
  * Errors: every function returns 0 (CHORUS_OK) or a negative code; chorus_last_error gives a message.
@@ -73,8 +74,9 @@ typedef struct {
  * order: 2..9.  cuda_stream: a cudaStream_t (NULL = default stream).  *out is NULL on failure. */
 int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chorus_physics* phys, void* cuda_stream);
 void chorus_free(chorus_ctx* ctx);
-/* Replace the physical parameters (e.g. C_h once the initial wave speed is known).  Changing kr_scale
- * re-evaluates kappa_r at the flux points. */
+/* Replace the physical parameters (e.g. C_h once the initial wave speed is known).  The kappa_r profile (kr_scale, kr_c,
+ * kr_wscale) is tabulated at the flux points by chorus_init and is fixed for the life of the context: a call that
+ * changes any of them returns CHORUS_EINVAL and leaves the context unchanged. */
 int chorus_set_physics(chorus_ctx* ctx, const chorus_physics* phys);
 
 /* q: [9][n_elem][n^3] fp64, HOST (on_device = 0) or DEVICE (on_device = 1) pointer. */

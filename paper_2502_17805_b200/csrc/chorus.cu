@@ -301,6 +301,14 @@ struct Hot {
   }
 };
 
+// CHORUS_ONLY_ORDER=<n> (a build option of build.py, off by default) instantiates the kernels of one order only.
+#ifdef CHORUS_ONLY_ORDER
+#define DISPATCH_N(c, expr)                                                                  \
+  [&]() -> int {                                                                             \
+    if ((c)->n == CHORUS_ONLY_ORDER) { using H = Hot<CHORUS_ONLY_ORDER>; return expr; }      \
+    return fail((c), CHORUS_EINVAL, "this build serves one order only (CHORUS_ONLY_ORDER)"); \
+  }()
+#else
 #define DISPATCH_N(c, expr)                                          \
   [&]() -> int {                                                     \
     switch ((c)->n) {                                                \
@@ -315,6 +323,7 @@ struct Hot {
       default: return fail((c), CHORUS_EINVAL, "order must be 2..9"); \
     }                                                                \
   }()
+#endif
 
 int run_geometry(chorus_ctx* c) {
   const int N1 = c->n + 1;
@@ -518,6 +527,12 @@ int chorus_step(chorus_ctx* c, double dt, int nstages) {
     return DISPATCH_N(c, H::stage(c, Qin, o, nullptr));
   };
   int rc = 0;
+  // a stage that fails leaves the trace buffers describing an intermediate state: they must not be reused
+  struct TraceGuard {
+    chorus_ctx* c;
+    bool ok = false;
+    ~TraceGuard() { if (!ok) c->traces_valid = false; }
+  } guard{c};
   if (nstages == 1) {
     if ((rc = run(b[0], b[1], U[b[0]], 1.0, nullptr, 0, nullptr, 0, dt))) return rc;
     c->cur = b[1];
@@ -544,6 +559,7 @@ int chorus_step(chorus_ctx* c, double dt, int nstages) {
     if ((rc = run(b[4], b[0], U[b[1]], c51, U[b[2]], c52, U[b[4]], a54, b54 * dt))) return rc;
     c->cur = b[0];
   }
+  guard.ok = true;
   return CHORUS_OK;
 }
 
@@ -679,17 +695,6 @@ int chorus_fp64_peak(int mode, double seconds, double* tflops, double* dfma_tflo
   if (dmma_tflops) *dmma_tflops = mode == 1 ? *tflops : mode == 2 ? 0.5 * *tflops : 0.0;
   return CHORUS_OK;
 }
-
-#ifdef CHORUS_PHASE_TIMING
-int chorus_debug_phase_cycles(unsigned long long* out16, int reset) {
-  if (out16 && cudaMemcpyFromSymbol(out16, g_phase_cycles, sizeof(unsigned long long) * 16) != cudaSuccess) return CHORUS_ECUDA;
-  if (reset) {
-    unsigned long long z[16] = {0};
-    if (cudaMemcpyToSymbol(g_phase_cycles, z, sizeof z) != cudaSuccess) return CHORUS_ECUDA;
-  }
-  return CHORUS_OK;
-}
-#endif
 
 int chorus_get_operators(int order, double* xs, double* xf, double* Isf, double* Dfs) {
   if (order < 2 || order > kMaxN) return CHORUS_EINVAL;

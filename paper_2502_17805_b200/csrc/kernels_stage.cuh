@@ -213,10 +213,6 @@ __device__ __forceinline__ void vs_flux_wall(const PhysD& ph, int wall, const VS
   Fv[3] = -qn + res;
 }
 
-#ifndef CHORUS_MAIN_MINBLOCKS
-#define CHORUS_MAIN_MINBLOCKS 2
-#endif
-
 // first k-step of a product: D = A*B (accumulator starts at zero, no register zeroing)
 __device__ __forceinline__ void dmma884z(double& d0, double& d1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%4};\n"
@@ -254,14 +250,9 @@ __device__ __forceinline__ void tma_load(void* smem, const void* gmem, unsigned 
                "l"(gmem), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(mb))
                : "memory");
 }
-// Not needed on the load path: every generic-proxy access to a destination buffer has been performed and observed by other
-// threads (barrier-ordered) before the bulk copy that overwrites it is issued -- the consumer-release -> producer-load pattern.
-// (Measured cost when issued by a thread with global stores in flight: ~1k cycles.)  -DCHORUS_PROXY_FENCE puts it back.
-__device__ __forceinline__ void fence_proxy_async() {
-#ifdef CHORUS_PROXY_FENCE
-  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-#endif
-}
+// Orders the generic-proxy accesses of a destination buffer (made by other threads and ordered before this point by a barrier)
+// before the async-proxy writes of the bulk copy that overwrites it: issued by every thread that issues a bulk copy.
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];\n" ::"l"(p)); }
 // all threads of the CTA: prefetch `bytes` starting at p into L2, one request per 128-byte line
@@ -286,13 +277,10 @@ template <int N> struct MainCfg {
 };
 // 128 * (chain + helper) = the CTA's 256 * 128 registers: two CTAs per SM.  With diffusion the chain warps carry the streamed
 // viscous flux state and need 160; without it they are light and the helpers (sources, RK, next-state traces) get the room.
-#ifndef CHORUS_NODIFF_CHAIN_REGS
-#define CHORUS_NODIFF_CHAIN_REGS 144
-#endif
 template <bool DIFF, int CWG = 1> struct RegSplit {
   // one chain warpgroup: launch at 128 registers (two CTAs per SM); two: launch at 168 (one CTA), 2 x 200 + 96 <= 3 x 168
   static constexpr int kLaunch = CWG == 2 ? 168 : 128;
-  static constexpr int kChain = CWG == 2 ? 200 : DIFF ? 160 : CHORUS_NODIFF_CHAIN_REGS;
+  static constexpr int kChain = CWG == 2 ? 200 : DIFF ? 160 : 144;
   static constexpr int kHelp = CWG == 2 ? 96 : 256 - kChain;
 };
 
@@ -367,7 +355,9 @@ __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, c
 // chain rule and the first interpolations) are awaited here, just before they are needed, and the left-over direction-0
 // points of sR are zeroed.
 // STORE: 1 store the divergence contribution, 0 accumulate it, -1 (default): store for direction 0, accumulate otherwise.
-template <int N, bool DIFF, int D, bool WAITF = false, int STORE = -1>
+// SYNCB: this is the warp's first task of a round that accumulates: the chain-warp barrier that separates the rounds is taken
+// here, just before the update, instead of before the task (the warps drift apart by less than the barrier used to cost).
+template <int N, bool DIFF, int D, bool WAITF = false, int STORE = -1, bool SYNCB = false>
 __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, const ElemNbr& nb, const StageIO& io, const Geo& geo,
                                           int64_t e, const double* sQ, const double* sG, const double* sFace, const double* sS, double* sR,
                                           int ln, bool lv, int dd = 0, int ctid = 0) {
@@ -519,6 +509,7 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
   for (int v = 0; v < 9; ++v) dmma884z(r0[v], r1[v], q0[v], L.bD0);
 #pragma unroll
   for (int v = 0; v < 9; ++v) dmma884(r0[v], r1[v], q1[v], L.bD1);
+  if (SYNCB) bar_sync(kBarChain, 128 * Mma<N>::kChainWG);     // every update of the previous round is in sR
 #pragma unroll
   for (int v = 0; v < 9; ++v) {
     constexpr bool kStore = STORE == 1 || (STORE == -1 && D == 0);
@@ -546,20 +537,6 @@ __device__ __forceinline__ void prefetch_next(const StageIO& io, const Geo& geo,
     for (size_t o = 0; o < sizeof(double) * 9 * I::n2; o += 128) prefetch_l2(b + o);
   }
 }
-
-#ifdef CHORUS_PHASE_TIMING   // development aid: per-phase clock cycles of the first chain thread of every CTA, summed into g_phase_cycles
-__device__ unsigned long long g_phase_cycles[16];
-#define CHORUS_TICK(k)                                                              \
-  do {                                                                              \
-    if (threadIdx.x == 0) {                                                         \
-      const long long t_ = clock64();                                               \
-      atomicAdd(&g_phase_cycles[k], (unsigned long long)(t_ - tick_));              \
-      tick_ = t_;                                                                   \
-    }                                                                               \
-  } while (0)
-#else
-#define CHORUS_TICK(k) do { } while (0)
-#endif
 
 // GRADV: 0 no gradient needed, 1 gradient of B only (Powell sources without diffusion), 2 all nine variables.
 //
@@ -684,12 +661,8 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     // arriving on an SM starts half a turn ahead
     int tail_rot = s_second ? M::kWarps / 2 : 0;
     constexpr int P2 = (I::n3 + CH - 1) / CH;     // solution points per chain thread in the chain rule
-#ifdef CHORUS_PHASE_TIMING
-    long long tick_ = clock64();
-#endif
     unsigned ld_phase = 0;
     for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
-      CHORUS_TICK(0);
       int tw = M::kWarps, tl_d = 0, tl_ln = 0;
       bool tl_ok = false;
       if (M::kTail > 0 && active) {
@@ -700,21 +673,22 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         tl_ln = M::line_of(tl_d, 8 * M::FG + (tl_ok ? q % (M::LO > 0 ? M::LO : 1) : 0));
         tail_rot = (tail_rot + 1) % M::kWarps;
       }
-      // chain-rule metrics of this thread's solution points: issued now, consumed after the gradient DMMAs
       double jv[P2][9];
-      if (GRADV != 0) {
+      auto load_jv = [&]() {     // chain-rule metrics of this thread's solution points (L2-resident: prefetched an element ahead)
+        if (GRADV != 0) {
 #pragma unroll
-        for (int q = 0; q < P2; ++q) {
-          const int s = tid + q * CH;
-          const int sc = s < I::n3 ? s : 0;
+          for (int q = 0; q < P2; ++q) {
+            const int s = tid + q * CH;
+            const int sc = s < I::n3 ? s : 0;
 #pragma unroll
-          for (int k = 0; k < 9; ++k) jv[q][k] = geo.jinv[e * 9 * I::n3 + k * I::n3 + sc];
+            for (int k = 0; k < 9; ++k) jv[q][k] = geo.jinv[e * 9 * I::n3 + k * I::n3 + sc];
+          }
         }
-      }
+      };
+      load_jv();                 // issued now, consumed after the gradient DMMAs
       if (kBulk) mbar_wait(&mbar, ld_phase);   // bulk copies: completion is observed by every consumer thread itself
       ld_phase ^= 1u;
       bar_sync(kBarIn, kMainThreads);          // inputs and wall states are in shared memory
-      CHORUS_TICK(1);
       // ---- A3: BR1 gradient.  d/dxi_d by DMMA, then the chain rule per point.
       if constexpr (GRADV != 0 && M::kFree) {
 #pragma unroll
@@ -733,7 +707,6 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         }
       }
       bar_sync(kBarGrad, kMainThreads);        // gradient DMMAs done (the helpers hold the face fluxes in registers)
-      CHORUS_TICK(2);
       if constexpr (GRADV != 0) {
 #pragma unroll
         for (int q = 0; q < P2; ++q) {
@@ -749,7 +722,6 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         }
       }
       bar_sync(kBarChain, CH);                  // the gradient is complete in shared memory
-      CHORUS_TICK(3);
       if constexpr (M::kFree) {
         // ---- A1, A4, A5, A7: every task stores into the accumulator of its own direction; no barrier between tasks
 #pragma unroll
@@ -769,28 +741,36 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         } else {
           bar_sync(kBarFaces, kMainThreads);
         }
-        bar_sync(kBarChain, CH);
-        CHORUS_TICK(4);
-        if (active) {
+        {   // rounds 1, 2 and the tail round: the round barrier sits inside the warp's first task of the round
+          bool first = true;
+          if (active) {
 #pragma unroll
-          for (int k = 0; k < M::kTPD; ++k)
-            if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
-        }
-        bar_sync(kBarChain, CH);
-        CHORUS_TICK(5);
-        if (active) {
+            for (int k = 0; k < M::kTPD; ++k)
+              if (warp + k * M::kWarps < M::FG) {
+                if (k == 0) chain_dir<N, DIFF, 1, false, -1, true>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
+                else chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
+                first = false;
+              }
+          }
+          if (first) bar_sync(kBarChain, CH);
+          first = true;
+          if (active) {
 #pragma unroll
-          for (int k = 0; k < M::kTPD; ++k)
-            if (warp + k * M::kWarps < M::FG) chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
-        }
-        if (M::kTail > 0) {   // left-over lines of the three directions: no two of them share a solution point
-          bar_sync(kBarChain, CH);
-          CHORUS_TICK(6);
-          if (active && tw < M::kTail) chain_dir<N, DIFF, 3>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, tl_ln, tl_ok, tl_d);
+            for (int k = 0; k < M::kTPD; ++k)
+              if (warp + k * M::kWarps < M::FG) {
+                if (k == 0) chain_dir<N, DIFF, 2, false, -1, true>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
+                else chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
+                first = false;
+              }
+          }
+          if (first) bar_sync(kBarChain, CH);
+          if (M::kTail > 0) {   // left-over lines of the three directions: no two of them share a solution point
+            if (active && tw < M::kTail) chain_dir<N, DIFF, 3, false, -1, true>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, tl_ln, tl_ok, tl_d);
+            else bar_sync(kBarChain, CH);
+          }
         }
       }
       bar_sync(kBarRes, kMainThreads);         // divergence accumulated: the helpers finish the element
-      CHORUS_TICK(7);
     }
   } else {
     // =============================================== helper warps ==============================================
@@ -820,11 +800,16 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           const bool whole = tid < 6 && pn_e >= 0 && pn_o == 0;
           const unsigned cnt = __popc(__ballot_sync(0xffffffffu, whole));
           if (tid == 0) {
+            fence_proxy_async();
             mbar_expect_tx(&mbar, (unsigned)(sizeof(double) * (9 * I::n3 + 9 * I::nf + cnt * 9 * I::n2)));
             tma_load(sQ, q, sizeof(double) * 9 * I::n3, &mbar);
           }
-          if (whole) tma_load(sQn + tid * 9 * I::n2, io.Qf + ((int64_t)pn_e * 6 + pn_f) * 9 * I::n2, sizeof(double) * 9 * I::n2, &mbar);
+          if (whole) {
+            if (tid != 0) fence_proxy_async();
+            tma_load(sQn + tid * 9 * I::n2, io.Qf + ((int64_t)pn_e * 6 + pn_f) * 9 * I::n2, sizeof(double) * 9 * I::n2, &mbar);
+          }
         } else if (tid == 32) {
+          fence_proxy_async();
           tma_load(sS, g, sizeof(double) * 9 * I::nf, &mbar);
         }
       } else {
@@ -846,6 +831,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       const double* t = io.Qf + el * 54 * I::n2;
       if (kBulk) {
         if (tid == 64) {
+          fence_proxy_async();
           mbar_expect_tx(&mbar, (unsigned)(sizeof(double) * 54 * I::n2));
           tma_load(sQo, t, sizeof(double) * 54 * I::n2, &mbar);
         }
@@ -958,9 +944,8 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           }
         }
       }
-#ifndef CHORUS_NO_L2_PREFETCH   // measured: -0.9k cycles of the 6.2k the chain warps wait for the next element's inputs
+      // measured: -0.9k cycles of the 6.2k the chain warps wait for the next element's inputs
       if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, pn_e, pn_f, tid, H);
-#endif
       bar_sync(kBarRes, kMainThreads);
 
       // ---- A9: finish the element.  The next element's state, metrics and neighbour traces start streaming in first

@@ -126,6 +126,35 @@ def test_p7_shear_resistive_and_thermal_decay_rates():
     np.testing.assert_allclose(r[4], -rate * eps * sx, rtol=0, atol=1e-5 * eps * rate)
 
 
+def test_p7_kappa_r_profile_on_the_shell():
+    """kappa_r(r) = kr_scale (c0 + c1 w + c2 w^2), w = r kr_wscale, tabulated at the flux points: with uniform
+    density, U = B = 0, kappa = 0 and T = T0 + eps r the energy row of Eq. 7, 9 leaves
+        dE/dt = div(kappa_r rho Cp grad T) = rho Cp eps [2 kappa_r(r)/r + kappa_r'(r)]
+    -- a closed form in which c1 and c2 swapped, kr_wscale dropped or r taken at the element centres are all O(1)
+    wrong (measured: 1.6, 0.53, ~0.1), while the discretisation error at n = 6 on 6x3x3x3 is 2.5e-4."""
+    n, nz, nr = 6, 3, 3
+    lam, c, ws = 0.02, (1.0, -0.8, 0.6), 1.7
+    R_gas = 1.3
+    Cp = GAM * R_gas / (GAM - 1)
+    m = I.cubed_sphere_shell(nz, nr, 0.7, 0.95, I.lobatto_abscissae(n + 1))
+    o = ob.Oracle(m, n, I.Physics(R_gas=R_gas, Cp=Cp, kr_scale=lam, kr_c=c, kr_wscale=ws, flags=I.FLAG_DIFFUSION))
+    x = o.geometry()["xsol"]
+    r = np.sqrt((x ** 2).sum(0))
+    rho0, T0, eps = 1.5, 1.0, 0.3
+    one, zero3 = np.ones_like(r), np.zeros((3,) + r.shape)
+    o.set_state(I.conserved(rho0 * one, zero3, rho0 * R_gas * (T0 + eps * r), zero3, 0 * one, GAM))
+    res = o.residual()
+    w = r * ws
+    kr = lam * (c[0] + c[1] * w + c[2] * w * w)
+    dkr = lam * ws * (c[1] + 2 * c[2] * w)
+    ref = rho0 * Cp * eps * (2 * kr / r + dkr)
+    layer = (np.arange(m["n_elem"]) % (nz * nz * nr)) // (nz * nz)
+    mid = layer == 1                                            # elements that touch no wall
+    assert np.abs(res[4][mid] - ref[mid]).max() <= 2e-3 * np.abs(ref[mid]).max()
+    # nothing else moves but momentum (p is not uniform): only the round-off of the Rusanov jump terms
+    assert np.abs(res[0]).max() <= 1e-10 and np.abs(res[5:]).max() <= 1e-10
+
+
 # ------------------------------------------------------------------------------- BR1 gradient
 def test_p8_gradient_exact_for_polynomials_and_spectral_on_shell():
     n = 5

@@ -235,4 +235,7 @@ def test_source_terms():
     M0, _ = ob.source(ph.copy(flags=0), Q, G, x)
     assert np.all(M0 == 0)
     Mc, _ = ob.source(ph.copy(flags=I.FLAG_CENTRIFUGAL), Q, G, x)
-    np.testing.assert_allclose(Mc[1:4], -rho * np.cross([0, 0, ph.Omega], np.cross([0, 0, ph.Omega], x)), atol=1e-14)
+    cen = -rho * np.cross([0, 0, ph.Omega], np.cross([0, 0, ph.Omega], x))          # -rho Omega x (Omega x x)  (reading G22)
+    np.testing.assert_allclose(Mc[1:4], cen, atol=1e-14)
+    np.testing.assert_allclose(Mc[4], u @ cen, atol=1e-14)                            # its work term, the energy row
+    assert Mc[0] == 0.0 and np.all(Mc[5:] == 0.0)

@@ -380,7 +380,8 @@ class Workload:
 
 
 def workload(name: str) -> Workload:
-    """configs[0..3] of BASELINE.json and the order sweep configs[4] ('sweep_n4' .. 'sweep_n9')."""
+    """configs[0..3] of BASELINE.json and the order sweep configs[4] ('sweep_n4' .. 'sweep_n9' at N_rho = 3, 'sweep1_n4' ..
+    'sweep1_n9' at N_rho = 1)."""
     sh1, sh3 = Shell(N_rho=1.0), Shell(N_rho=3.0)
     table = {
         "config0": Workload("config0", 6, 4, 2, 1.0, 0, 0.0, True, 2, sh1),
@@ -395,6 +396,10 @@ def workload(name: str) -> Workload:
         "sweep_n8": Workload("sweep_n8", 8, 22, 7, 3.0, 4, 1e-3, True, 2, sh3),
         "sweep_n9": Workload("sweep_n9", 9, 18, 7, 3.0, 4, 1e-3, True, 2, sh3),
     }
+    # configs[4] asks for N_rho = 1 and 3: the same meshes on the shallower polytrope
+    for n in range(4, 10):
+        w3_ = table[f"sweep_n{n}"]
+        table[f"sweep1_n{n}"] = Workload(f"sweep1_n{n}", n, w3_.n_z, w3_.n_r, 1.0, 4, 1e-3, True, 2, sh1)
     return table[name]
 
 

@@ -23,7 +23,7 @@ def g24_error(r_test, r_ref, a_ref):
     """Per-variable max |dR| / max A (magnitude residual of the reference): forward-error norm of reading G24."""
     d = np.abs(r_test - r_ref).reshape(9, -1).max(1)
     den = a_ref.reshape(9, -1).max(1)
-    den = np.maximum(den, 1e-3 * den.max())     # rows whose every term is round-off (e.g. psi = 0) use the global scale
+    den = np.where(den > 0.0, den, den.max())   # only a row whose every term is identically zero borrows the global scale
     return d / den
 
 

@@ -155,6 +155,23 @@ def test_order_sweep_parity(n, diff):
     assert g25_error(g.get_state(), o.get_state(), phys.c_h).max() <= STATE_TOL
 
 
+@pytest.mark.parametrize("n,diff", [(4, 1e-3), (4, 0.0), (5, 1e-3), (5, 0.0), (6, 1e-3), (6, 0.0), (7, 1e-3), (7, 0.0)])
+def test_persistent_loop_parity(n, diff):
+    """Meshes with more elements (6x8x8x2 = 768) than the element kernel's grid (2 CTAs x 148 SMs, 1 x 148 at n = 7), so that
+    every CTA runs its persistent loop several times -- barrier phases, bulk copies into live shared memory, tail-task rotation,
+    the new state passing through sQ for its traces -- in RESIDUAL and in STEP mode, against the whole-mesh oracle."""
+    w, mesh, o, g, Q, phys = shell_case(n, 8, 2, 3.0, 12, diff)
+    assert mesh["n_elem"] == 768
+    check_residual(o, g)
+    _, xf, _, _ = P.get_operators(n)
+    dt = w.dt(o.max_wavespeed(), xf[1] - xf[0])
+    for _ in range(2):
+        o.step(dt, 5); g.step(dt, 5)
+    err = g25_error(g.get_state(), o.get_state(), phys.c_h)
+    assert err.max() <= STATE_TOL, err
+    check_residual(o, g)
+
+
 @pytest.mark.parametrize("nstages", [1, 3])
 def test_other_rk_schemes_parity(nstages):
     w, mesh, o, g, Q, phys = shell_case(4, 3, 2, 1.0, 9, 1e-3)

@@ -26,58 +26,92 @@ import numpy as np  # noqa: E402
 METRIC = "SD-MHD DOF-updates/s (sol pts x 9 vars x RK stages)"
 UNIT = "DOF-updates/s"
 NSTAGES = 5
-# Algorithmic work per solution point per RK stage at n = 6 (restated in DESIGN.md 7.3), keyed by
-# "diffusion on": HBM bytes (whole stage, element kernel's share) and flop (whole stage, element kernel's share).
-ALG_BYTES = {True: (660.0, 532.0), False: (548.0, 548.0)}
-ALG_FLOPS = {True: (3550.0, 3360.0), False: (1370.0, 1370.0)}
-# Other orders, full physics: n -> (flop, bytes) per point per stage, whole stage.
+# Algorithmic work per solution point per RK stage: the MODEL of SURVEY.md S8(d) / Appendix A5 (restated in DESIGN.md 7.3 and
+# BASELINE.md 3), not an operation tally of the kernels.  Full physics, whole stage: n -> (flop, bytes).
 ALG_BY_ORDER = {4: (3008.0, 794.0), 5: (3267.0, 714.0), 6: (3550.0, 660.0), 7: (3840.0, 622.0), 8: (4141.0, 593.0), 9: (4447.0, 571.0)}
+# The viscous face kernel's part of it, the same for every order per point up to the 6/n face points per point:
+# 190 flop (108 for the next state's face traces, 54 n^3 FMA per element; 82 for the face correction, 7 components x 6 FMA)
+# and 128 B x 6/n (own + neighbour face viscous fluxes, 14 words per face point, and |J|).
+FACE_FLOPS, FACE_BYTES_N6 = 190.0, 128.0
 
 
 def alg_work(n, diff):
-    """((stage_bytes, kernel_bytes), (stage_flops, kernel_flops)) per solution point per stage for order n.
-    The element kernel's share of the stage is scaled from the n = 6 split (the rest is the viscous face kernel: face
-    correction and next traces); without diffusion only the n = 6 figures exist and are scaled by the full-physics ratio."""
-    if n == 6:
-        return ALG_BYTES[diff], ALG_FLOPS[diff]
+    """((stage_bytes, kernel_bytes), (stage_flops, kernel_flops)) per solution point per stage for order n; "kernel" is the
+    element kernel (the dominant one).  Diffusion off, Powell sources on (configs 0, 2): contraction FMA x 2 =
+    2 [2 x 27 (n+1) + 3 (3 (n+1) + 9)] plus the pointwise work of the n = 6 model (434 flop) scaled with the flux points per
+    point; bytes = the full-physics figure minus the face viscous traces (2 x 7 x 6/n words)."""
     f, b = ALG_BY_ORDER.get(n, ALG_BY_ORDER[6])
     if not diff:
-        f, b = f * 1370.0 / 3550.0, b * 548.0 / 660.0
+        f = 2.0 * (54.0 * (n + 1) + 3.0 * (3.0 * (n + 1) + 9.0)) + 434.0 * ((n + 1) / n) / (7.0 / 6.0)
+        b = b - 8.0 * 14.0 * 6.0 / n
         return (b, b), (f, f)
-    return (b, b * 532.0 / 660.0), (f, f * 3360.0 / 3550.0)
+    return (b, b - FACE_BYTES_N6 * 6.0 / n), (f, f - FACE_FLOPS)
+
+
 FP64_PEAK_TFLOPS = 37.2   # 148 SMs x 4 sub-partitions x 16 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7.3; DMMA measured 37.0)
 
 
-def cpu_sample_workload(w):
-    """Bounded sample of the same workload for the CPU oracle: same order, physics, generator; fewer elements."""
+def cpu_sample_workload(w, n_r=8):
+    """Bounded sample of the same workload for the CPU oracle: same order, physics, polytrope and generator on a
+    6 x 16 x 16 x n_r shell (n_r = 8: 12,288 elements; the whole of config 3 needs 30 GB and minutes per step on the host)."""
     from paper_2502_17805_b200 import inputs as I
-    return I.Workload(w.name + "-cpu-sample", w.order, 16, 6, w.N_rho, w.seed, w.diffusion, w.dipole, shell=w.shell)
+    return I.Workload(w.name + "-cpu-sample", w.order, 16, n_r, w.N_rho, w.seed, w.diffusion, w.dipole, shell=w.shell)
 
 
-def time_oracle(w, steps, warmup):
-    """Oracle (as it stands) on the host cores: DOF-updates/s over `steps` SSPRK(5,3) steps of the sample."""
+def omp_threads(n=None):
+    """Thread count of the oracle's OpenMP runtime (set it when n is given)."""
+    import ctypes
+    try:
+        gomp = ctypes.CDLL("libgomp.so.1")
+        if n is not None:
+            gomp.omp_set_num_threads(int(n))
+        return int(gomp.omp_get_max_threads())
+    except OSError:
+        return int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+
+
+def time_oracle(w, steps, warmup, n_r=8, threads=None):
+    """Oracle (as it stands) on the host cores: DOF-updates/s over `steps` SSPRK(5,3) steps of the sample, after `warmup`
+    untimed steps (0: one untimed residual evaluation instead, which spins up the thread team and touches the arrays)."""
     from oracle import binding as ob
     from paper_2502_17805_b200 import inputs as I
-    ws = cpu_sample_workload(w)
+    ws = cpu_sample_workload(w, n_r)
     mesh = ws.mesh()
-    o = ob.Oracle(mesh, ws.order, I.Physics())
-    Q = ws.state(o.geometry()["xsol"])
-    o.set_state(Q)
-    c_h = o.max_wavespeed()
-    o.set_physics(ws.physics(c_h))
-    _, xf = ob.nodes(ws.order)
-    dt = ws.dt(c_h, xf[1] - xf[0])
-    for _ in range(warmup):
-        o.step(dt, NSTAGES)
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        o.step(dt, NSTAGES)
-    t = time.perf_counter() - t0
+    all_threads = omp_threads()
+    cores = omp_threads(threads) if threads else all_threads
+    try:
+        o = ob.Oracle(mesh, ws.order, I.Physics())
+        Q = ws.state(o.geometry()["xsol"])
+        o.set_state(Q)
+        c_h = o.max_wavespeed()
+        o.set_physics(ws.physics(c_h))
+        _, xf = ob.nodes(ws.order)
+        dt = ws.dt(c_h, xf[1] - xf[0])
+        if warmup == 0:
+            o.residual()
+        for _ in range(warmup):
+            o.step(dt, NSTAGES)
+        per_step = []
+        for _ in range(steps):
+            t0 = time.perf_counter()
+            o.step(dt, NSTAGES)
+            per_step.append(time.perf_counter() - t0)
+    finally:
+        if threads:
+            omp_threads(all_threads)
     pts = mesh["n_elem"] * ws.order ** 3
-    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    return dict(value=pts * 9 * NSTAGES * steps / t, unit=UNIT, cores=cores, kind="oracle",
-                sample=f"{steps} SSPRK(5,3) step(s) of the 6x{ws.n_z}x{ws.n_z}x{ws.n_r} = {mesh['n_elem']}-element shell, order {ws.order}, "
-                       f"same physics and generator as {w.name}", seconds=t), t / steps
+    t_med = float(np.median(per_step))
+    return dict(value=pts * 9 * NSTAGES / t_med, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"median of {steps} SSPRK(5,3) step(s) of the 6x{ws.n_z}x{ws.n_z}x{ws.n_r} = {mesh['n_elem']}-element shell, order "
+                       f"{ws.order}, same physics, polytrope and generator as {w.name}", seconds=float(sum(per_step))), t_med
+
+
+def workload_config(w, args, world, pts=None):
+    """The `config` object of the JSON line: identical for both arms (the reference arm's sample is named in cpu_baseline)."""
+    pts = w.n_elem * w.order ** 3 if pts is None else pts
+    return dict(workload=args.workload, mesh=f"6x{w.n_z}x{w.n_z}x{w.n_r} cubed-sphere shell", n_elem=w.n_elem, order=w.order,
+                solution_points=pts, N_rho=w.N_rho, diffusion=w.diffusion, rk="SSPRK(5,3)",
+                parallelism="replicas" if world > 1 else "single GPU", l2="inputs larger than L2 (state %.0f MB)" % (pts * 72 / 1e6))
 
 
 class ClockSampler:
@@ -156,18 +190,19 @@ def ncu_traffic(workload):
 
 
 def run_reference(args, rank, world):
-    """--impl reference: the oracle, as it stands, on the box's host cores (rank 0 only)."""
+    """--impl reference: the oracle, as it stands, on the box's host cores (rank 0 only).  Every one of the --steps K steps is
+    one SSPRK(5,3) step of a bounded sample of the workload, sized so that K + W steps end within a few minutes."""
     if rank != 0:
         return
     from paper_2502_17805_b200 import inputs as I
     w = I.workload(args.workload)
-    steps = max(1, min(args.steps, 10))
-    cb, sec_per_step = time_oracle(w, steps, min(args.warmup, 3))
-    line = dict(impl="reference", metric=METRIC, value=cb["value"], unit=UNIT, n_gpus=args.gpus, steps=steps, warmup=min(args.warmup, 3),
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    n_r = 8 if steps + warmup <= 8 else 4 if steps + warmup <= 16 else 2 if steps + warmup <= 32 else 1
+    cb, sec_per_step = time_oracle(w, steps, warmup, n_r=n_r)
+    cb.pop("seconds", None)
+    line = dict(impl="reference", metric=METRIC, value=cb["value"], unit=UNIT, n_gpus=args.gpus, steps=steps, warmup=warmup,
                 ms_per_step=1e3 * sec_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
-                data="synthetic", config=dict(workload=args.workload, sample=cb["sample"], order=w.order,
-                                              parallelism="host cores (OpenMP over elements)"),
-                cpu_baseline=dict(value=cb["value"], unit=UNIT, cores=cb["cores"], kind="oracle", sample=cb["sample"]),
+                data="synthetic", config=workload_config(w, args, world), cpu_baseline=cb,
                 e2e=dict(value=cb["value"], unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
     print(json.dumps(line), flush=True)
 
@@ -227,12 +262,10 @@ def main():
     # ---- device-resident throughput
     for _ in range(warmup):
         g.step(dt, NSTAGES)
-    g.profile(True)
-    g.profile_read()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = g.launch_count()
     barrier()
-    with ClockSampler(local) as clocks:
+    with ClockSampler(local) as clocks:     # the headline loop: no per-launch events
         ev0.record()
         for _ in range(args.steps):
             g.step(dt, NSTAGES)
@@ -240,25 +273,44 @@ def main():
         barrier()
     ms = ev0.elapsed_time(ev1)
     launches = g.launch_count() - l0
+    ws_after = g.max_wavespeed()          # also proves the state is still finite
+    # ---- per-kernel device times: a separate pass with every launch bracketed by CUDA events on the library's stream
+    g.profile(True)
+    g.profile_read()
+    prof_steps = max(1, min(args.steps, 4))
+    for _ in range(prof_steps):
+        g.step(dt, NSTAGES)
     prof = g.profile_read()
     g.profile(False)
-    ws_after = g.max_wavespeed()          # also proves the state is still finite
+    prof_ms = sum(v[0] for v in prof.values())
     # ---- end to end through the C ABI with HOST buffers: H2D of the state, one step, D2H of the CFL wave speed
-    e2e_ms, e2e_steps = None, 0
+    # Every step: H2D of the state from pinned memory, one step, D2H of the new state into pinned memory, the CFL wave speed.
+    e2e_ms, e2e_nod2h_ms, e2e_steps = None, None, 0
     if not args.no_e2e:
         e2e_steps = max(1, min(args.steps, 5))
         hnp = host.numpy()
-        g.set_state(hnp); g.step(dt, NSTAGES); g.max_wavespeed()
+        out = torch.empty_like(host).pin_memory().numpy()
+        g.set_state(hnp); g.step(dt, NSTAGES); g.get_state(out); g.max_wavespeed()
         barrier()
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
             g.set_state(hnp)
             g.step(dt, NSTAGES)
+            g.get_state(out)
             g.max_wavespeed()
         barrier()
         e2e_ms = 1e3 * (time.perf_counter() - t0)
-    ms, e2e_max = max_over_ranks([ms, e2e_ms or 0.0], dist)
-    e2e_ms = e2e_max if e2e_ms is not None else None
+        assert np.isfinite(out[:, ::max(1, out.shape[1] // 64)]).all()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):          # the same without the state coming back (round 1's figure), for comparison
+            g.set_state(hnp)
+            g.step(dt, NSTAGES)
+            g.max_wavespeed()
+        barrier()
+        e2e_nod2h_ms = 1e3 * (time.perf_counter() - t0)
+    ms, e2e_max, e2e_nod2h_max = max_over_ranks([ms, e2e_ms or 0.0, e2e_nod2h_ms or 0.0], dist)
+    if e2e_ms is not None:
+        e2e_ms, e2e_nod2h_ms = e2e_max, e2e_nod2h_max
     peaks = None
     if rank == 0:   # sustained FP64 issue rates of this device (DFMA, DMMA), ~0.5 s each: the "alu" roofline's measured companion
         try:
@@ -283,17 +335,19 @@ def main():
     t_alu = stage_flops * pts / (FP64_PEAK_TFLOPS * 1e12) * 1e3
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=warmup, ms_per_step=ms / args.steps,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
-                config=dict(workload=args.workload, mesh=f"6x{w.n_z}x{w.n_z}x{w.n_r} cubed-sphere shell", n_elem=g.E, order=n,
-                            solution_points=pts, N_rho=w.N_rho, diffusion=w.diffusion, rk="SSPRK(5,3)",
-                            parallelism="replicas" if world > 1 else "single GPU", l2="inputs larger than L2 (state %.0f MB)" % (pts * 72 / 1e6)),
+                config=workload_config(w, args, world, pts),
                 clocks=clocks.summary(), gpu_launches=launches,
                 roofline=dict(bound="alu", kernel="stage_main_kernel" if 4 <= n <= 7 else "residual_kernel", achieved=achieved, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
                               frac=(achieved / FP64_PEAK_TFLOPS) if achieved else None, traffic=ncu_traffic(args.workload),
+                              traffic_source="dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu --set full "
+                                             "capture (profiles/roofline_traffic.md); not measured in this run",
+                              alg_source="model of SURVEY.md S8(d) / Appendix A5 (BASELINE.md 3), not an operation tally",
                               peak_source="nominal FP64 pipe: 148 SMs x 4 x 16 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7.3)",
                               measured_fp64=peaks, alg_flops_per_point=kernel_flops, alg_bytes_per_point=kernel_bytes,
                               kernel_hbm=dict(achieved_gbs=kernel_bytes * pts / (main_avg_ms * 1e-3) / 1e9 if main_cnt else None,
                                               peak_gbs=hbm_peak, peak_source=peak_src),
-                              kernel_ms=kernel_ms, kernel_share_of_step={k: v[0] / ms for k, v in prof.items()},
+                              kernel_ms=kernel_ms, kernel_share_of_step={k: v[0] / prof_ms for k, v in prof.items()} if prof_ms else None,
+                              kernel_timing=f"separate pass of {prof_steps} step(s) with per-launch CUDA events; the headline loop runs without them",
                               stage=dict(ms=stage_ms, alg_bytes_per_point=stage_bytes, alg_flops_per_point=stage_flops,
                                          t_hbm_ms=t_hbm, t_alu_ms=t_alu, binding="alu" if t_alu >= t_hbm else "hbm",
                                          frac_of_binding=max(t_hbm, t_alu) / stage_ms,
@@ -302,11 +356,17 @@ def main():
                 wavespeed_after=ws_after)
     if e2e_ms is not None:
         line["e2e"] = dict(value=world * dof_per_step * e2e_steps / (e2e_ms * 1e-3), unit=UNIT, h2d_bytes_per_step=pts * 72,
-                           d2h_bytes_per_step=8, steps=e2e_steps, ms_per_step=e2e_ms / e2e_steps,
-                           what="chorus_set_state(pinned host) + chorus_step(dt,5) + chorus_max_wavespeed")
+                           d2h_bytes_per_step=pts * 72 + 8, steps=e2e_steps, ms_per_step=e2e_ms / e2e_steps,
+                           what="chorus_set_state(pinned host) + chorus_step(dt,5) + chorus_get_state(pinned host) + chorus_max_wavespeed",
+                           without_state_d2h=dict(value=world * dof_per_step * e2e_steps / (e2e_nod2h_ms * 1e-3),
+                                                  ms_per_step=e2e_nod2h_ms / e2e_steps, d2h_bytes_per_step=8))
     if world == 1 and not args.no_cpu_baseline:
-        cb, _ = time_oracle(w, 3, 0)      # ~10-20 s of host work on the box's cores
+        # the oracle on a 12,288-element sample of the same workload: one untimed residual, then one step on all cores
+        # (~20-40 s of host work), and one step of a 1,536-element sample on one core
+        cb, _ = time_oracle(w, 1, 0, n_r=8)
         cb.pop("seconds", None)
+        one, _ = time_oracle(w, 1, 0, n_r=1, threads=1)
+        cb["one_core"] = dict(value=one["value"], unit=UNIT, cores=one["cores"], sample=one["sample"])
         line["cpu_baseline"] = cb
     print(json.dumps(line), flush=True)
     if dist is not None:

@@ -96,6 +96,12 @@ int chorus_step(chorus_ctx* ctx, double dt, int nstages);
  * maximised over direction, for the CFL condition.  Synchronises.  CHORUS_ESTATE if it is not finite. */
 int chorus_max_wavespeed(chorus_ctx* ctx, double* out);
 
+/* Volume-averaged diagnostics of the current state: out (HOST, 3 doubles) =
+ *   V    = int dV,   KE = (1/V) int 1/2 rho U.U dV  (Eq. 34),   E_B = (1/V) int 1/2 B.B dV  (Eq. 35),
+ * with the interpolatory quadrature of the solution points, int f dV = sum_e sum_ijk w_i w_j w_k |J| f (w = Fejer's first rule
+ * on the Chebyshev-Gauss points of Eq. 18).  A deterministic two-kernel tree reduction; synchronises.  CHORUS_ESTATE without a state. */
+int chorus_diagnostics(chorus_ctx* ctx, double* out);
+
 const char* chorus_last_error(const chorus_ctx* ctx);
 
 /* ---- accessors used by the parity tests and by input generation (not on the hot path) ---- */

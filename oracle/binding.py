@@ -52,6 +52,8 @@ def lib():
         L.oracle_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.oracle_get_geometry.argtypes = [C.c_void_p] + [C.c_void_p] * 4
         L.oracle_nodes.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
+        L.oracle_quadrature_weights.argtypes = [C.c_int, C.c_void_p]
+        L.oracle_diagnostics.argtypes = [C.c_void_p, C.c_void_p]
         L.oracle_operators.argtypes = [C.c_int] + [C.c_void_p] * 4
         L.oracle_rk_tableau.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
         P, V = C.POINTER(_Phys), C.c_void_p
@@ -64,7 +66,9 @@ def lib():
         L.oracle_wavespeed.restype = C.c_double
         L.oracle_wall_state.argtypes = [P, C.c_int, V, V, V]
         L.oracle_flux_wall_inviscid.argtypes = [P, V, V, V]
-        L.oracle_flux_wall_viscous.argtypes = [P, C.c_int, V, V, V, C.c_double, V]
+        L.oracle_flux_wall_viscous.argtypes = [P, C.c_int, V, V, V, C.c_double, C.c_double, V]
+        L.oracle_wall_condition_gradB.argtypes = [C.c_int, V, V, V, C.c_double, V]
+        L.oracle_wall_condition_gradB.restype = None
         L.oracle_source.argtypes = [P, V, V, V, V, V]
         for f in ("oracle_flux_inviscid", "oracle_flux_viscous", "oracle_flux_rusanov", "oracle_wall_state",
                   "oracle_flux_wall_inviscid", "oracle_flux_wall_viscous", "oracle_source"):
@@ -86,6 +90,12 @@ def nodes(n):
     xs, xf = np.empty(n), np.empty(n + 1)
     assert lib().oracle_nodes(n, _p(xs), _p(xf)) == 0
     return xs, xf
+
+
+def quadrature_weights(n):
+    w = np.empty(n)
+    assert lib().oracle_quadrature_weights(n, _p(w)) == 0
+    return w
 
 
 def operators(n):
@@ -141,10 +151,18 @@ def flux_wall_inviscid(phys, Qb, nh):
     return F
 
 
-def flux_wall_viscous(phys, wall, Qb, G, nh, kr=0.0):
-    F = np.empty(9); Qb, G, nh = _d(Qb), _d(G), _d(nh)
-    lib().oracle_flux_wall_viscous(C.byref(physics_struct(phys)), wall, _p(Qb), _p(G), _p(nh), kr, _p(F))
+def flux_wall_viscous(phys, wall, Qb, G, nh, kr=0.0, rw=0.0):
+    F = np.empty(9)
+    Qb, G, nh = _d(Qb), _d(G), _d(nh)
+    lib().oracle_flux_wall_viscous(C.byref(physics_struct(phys)), wall, _p(Qb), _p(G), _p(nh), float(rw), float(kr), _p(F))
     return F
+
+
+def wall_condition_gradB(bc, dB, Bb, er, rw):
+    out = np.empty((3, 3))
+    dB, Bb, er = _d(dB), _d(Bb), _d(er)
+    lib().oracle_wall_condition_gradB(int(bc), _p(dB), _p(Bb), _p(er), float(rw), _p(out))
+    return out
 
 
 def source(phys, Q, G, x):
@@ -203,6 +221,12 @@ class Oracle:
         out = np.empty(1)
         assert lib().oracle_max_wavespeed(self._ctx, _p(out)) == 0
         return float(out[0])
+
+    def diagnostics(self):
+        """dict(V, KE, EB): shell volume, volume-averaged kinetic and magnetic energy (Eq. 34-35)."""
+        out = np.empty(3)
+        assert lib().oracle_diagnostics(self._ctx, _p(out)) == 0
+        return dict(V=float(out[0]), KE=float(out[1]), EB=float(out[2]))
 
     def gradient(self):
         g = np.empty((27, self.E, self.n ** 3))

@@ -102,6 +102,7 @@ void flux_inviscid_abs(const Phys<T>& ph, const T* Q, const T* S, T* F, bool wal
 template <class T>
 struct Visc {
   T tau[3][3], q[3], BxJ[3], dB[3][3];   // dB[i][j] = d_j B_i
+  T dT[3];                                 // grad T
 };
 template <class T>
 Visc<T> viscous_terms(const Phys<T>& ph, const Prim<T>& w, const T* G, T kr) {
@@ -133,6 +134,7 @@ Visc<T> viscous_terms(const Phys<T>& ph, const Prim<T>& w, const T* G, T kr) {
     for (int j = 0; j < 3; ++j) v.tau[i][j] = mu * (du[i][j] + du[j][i]) + (i == j ? lam * divu : T(0));   // Eq. 8
   T Tt = w.p / (w.rho * ph.R);
   for (int j = 0; j < 3; ++j) v.q[j] = -ph.kappa * w.rho * Tt * dS[j] - kr * w.rho * ph.Cp * dT[j];      // Eq. 9
+  for (int j = 0; j < 3; ++j) v.dT[j] = dT[j];
   T J[3] = {v.dB[2][1] - v.dB[1][2], v.dB[0][2] - v.dB[2][0], v.dB[1][0] - v.dB[0][1]};                  // J = curl B
   v.BxJ[0] = w.B[1] * J[2] - w.B[2] * J[1];
   v.BxJ[1] = w.B[2] * J[0] - w.B[0] * J[2];
@@ -208,27 +210,115 @@ void wall_state(const Phys<T>& ph, int wall, const T* Q, const T* nh, T* Qb) {
   Qb[4] = pb / (ph.gamma - T(1)) + T(0.5) * w.rho * (ub[0] * ub[0] + ub[1] * ub[1] + ub[2] * ub[2]) +
           T(0.5) * (Bb[0] * Bb[0] + Bb[1] * Bb[1] + Bb[2] * Bb[2]) + T(0.5) * w.psi * w.psi;   // Eq. 3
 }
+// Wall viscous flux along the outward unit normal nh from (Q_b, grad Q_in), with the wall conditions applied to the WALL
+// GRADIENTS as PAPER.md:198 describes ("transforming the Jacobian of the magnetic field into spherical coordinates and
+// setting the appropriate derivatives to zero"; stress tensor "converted to spherical coordinates, and the angular components
+// are set to zero"), reading G29 of DESIGN.md:
+//   frame     (e_r, t_1, t_2) at the wall point, e_r = the wall's radial direction = +nh on the outer wall, -nh on the inner
+//             wall (on the paper's spherical shells this is the spherical frame), r = rw = distance of the point from the origin;
+//             in this frame the spherical component derivatives are  d_r B_a = e_a.(dB/dr)  and, along a tangent t,
+//             d_t B_r = e_r.(dB/dt) + B_t/r,  d_s B_t = e_t.(dB/ds) - delta_st B_r/r  (the unit vectors turn with the position);
+//   conductor B_r = 0 on the whole surface, d_r(r B_t) = 0:   D[r][t] = -B_t/r (so that d_t B_r = 0),  D[t][r] = -B_t/r;
+//   radial    B_t = 0 on the whole surface, d_r(r^2 B_r) = 0:  D[s][t] = delta_st B_r/r (d_s B_t = 0),  D[r][r] = -2 B_r/r
+//             (the conditioned Jacobian is divergence free: "to maintain the divergence-free magnetic field");
+//   where D[a][b] = e_a.(grad B).e_b is the Cartesian Jacobian in the wall frame and B is the wall state's field.  The
+//   conditioned Jacobian gives the current J = curl B of the resistive terms only: grad p, grad T, grad S come from the
+//   unconditioned conserved gradients (conditioning grad B without grad E would change grad p);
+//   stress    tau_rt = tau_tr = 0 (stress-free);
+//   thermal   constant-temperature outer wall: T is uniform on the surface, the tangential part of grad T is zero;
+//             constant-flux inner wall: q.r_hat = q_bottom (Eq. 32).
+// rw <= 0 stands for a plane wall (1/r = 0).
 template <class T>
-void flux_wall_viscous(const Phys<T>& ph, int wall, const T* Qb, const T* G, const T* nh, T kr, T* F) {
+void wall_frame(const T* er, T R[3][3]) {          // columns of R: e_r, t_1, t_2 (right-handed, orthonormal)
+  int k = 0;                                       // Cartesian axis least aligned with e_r
+  for (int i = 1; i < 3; ++i)
+    if (std::fabs(er[i]) < std::fabs(er[k])) k = i;
+  T a[3] = {T(0), T(0), T(0)};
+  a[k] = T(1);
+  T t1[3] = {er[1] * a[2] - er[2] * a[1], er[2] * a[0] - er[0] * a[2], er[0] * a[1] - er[1] * a[0]};
+  T nrm = std::sqrt(t1[0] * t1[0] + t1[1] * t1[1] + t1[2] * t1[2]);
+  for (int i = 0; i < 3; ++i) t1[i] /= nrm;
+  T t2[3] = {er[1] * t1[2] - er[2] * t1[1], er[2] * t1[0] - er[0] * t1[2], er[0] * t1[1] - er[1] * t1[0]};
+  for (int i = 0; i < 3; ++i) { R[i][0] = er[i]; R[i][1] = t1[i]; R[i][2] = t2[i]; }
+}
+template <class T>
+void to_frame(const T R[3][3], const T A[3][3], T D[3][3]) {      // D = R^T A R
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b) {
+      T s = T(0);
+      for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) s += R[i][a] * A[i][j] * R[j][b];
+      D[a][b] = s;
+    }
+}
+template <class T>
+void from_frame(const T R[3][3], const T D[3][3], T A[3][3]) {    // A = R D R^T
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      T s = T(0);
+      for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) s += R[i][a] * D[a][b] * R[j][b];
+      A[i][j] = s;
+    }
+}
+// the conditioned Jacobian of B (dBc[i][j] = d_j B_i, Cartesian) of a wall with magnetic condition bc (0 conductor, 1 radial)
+template <class T>
+void wall_condition_gradB(int bc, const T dB[3][3], const T* Bb, const T* er, T rw, T dBc[3][3]) {
+  T R[3][3], D[3][3];
+  wall_frame(er, R);
+  to_frame(R, dB, D);
+  T ir = rw > T(0) ? T(1) / rw : T(0);
+  T Bl[3];                                         // wall-state field in the frame: (B_r, B_1, B_2)
+  for (int a = 0; a < 3; ++a) Bl[a] = Bb[0] * R[0][a] + Bb[1] * R[1][a] + Bb[2] * R[2][a];
+  if (bc == 0) {
+    for (int t = 1; t < 3; ++t) {
+      D[0][t] = -Bl[t] * ir;                       // d_t B_r = 0 on the surface
+      D[t][0] = -Bl[t] * ir;                       // d_r (r B_t) = 0
+    }
+  } else {
+    for (int s_ = 1; s_ < 3; ++s_)
+      for (int t = 1; t < 3; ++t) D[t][s_] = (s_ == t) ? Bl[0] * ir : T(0);   // d_s B_t = 0 on the surface
+    D[0][0] = -T(2) * Bl[0] * ir;                  // d_r (r^2 B_r) = 0
+  }
+  from_frame(R, D, dBc);
+}
+template <class T>
+void flux_wall_viscous(const Phys<T>& ph, int wall, const T* Qb, const T* G, const T* nh, T rw, T kr, T* F) {
   Prim<T> w = primitives(ph, Qb);
   Visc<T> v = viscous_terms(ph, w, G, kr);
   int bc = (wall == -1) ? ph.bc_inner : ph.bc_outer;
-  T t[3], tn = T(0);
-  for (int i = 0; i < 3; ++i) {
-    t[i] = v.tau[i][0] * nh[0] + v.tau[i][1] * nh[1] + v.tau[i][2] * nh[2];
-    tn += t[i] * nh[i];
+  T sgn = (wall == -1) ? T(-1) : T(1);
+  T er[3] = {sgn * nh[0], sgn * nh[1], sgn * nh[2]};
+  T R[3][3];
+  wall_frame(er, R);
+  // stress-free: angular components of the stress tensor in the wall frame set to zero
+  T tl[3][3], tc[3][3];
+  to_frame(R, v.tau, tl);
+  for (int t = 1; t < 3; ++t) tl[0][t] = tl[t][0] = T(0);
+  from_frame(R, tl, tc);
+  // magnetic wall: conditioned Jacobian of B, its current density
+  T dBc[3][3];
+  wall_condition_gradB(bc, v.dB, w.B, er, rw, dBc);
+  T J[3] = {dBc[2][1] - dBc[1][2], dBc[0][2] - dBc[2][0], dBc[1][0] - dBc[0][1]};
+  T BxJ[3] = {w.B[1] * J[2] - w.B[2] * J[1], w.B[2] * J[0] - w.B[0] * J[2], w.B[0] * J[1] - w.B[1] * J[0]};
+  // thermal walls
+  T q[3] = {v.q[0], v.q[1], v.q[2]};
+  if (wall == -2 && (ph.flags & F_TTOP)) {         // uniform T on the surface: only the radial part of grad T conducts
+    T dTr = v.dT[0] * er[0] + v.dT[1] * er[1] + v.dT[2] * er[2];
+    for (int j = 0; j < 3; ++j) q[j] += kr * w.rho * ph.Cp * (v.dT[j] - dTr * er[j]);
   }
-  for (int c = 0; c < 9; ++c) F[c] = T(0);
-  for (int i = 0; i < 3; ++i) F[1 + i] = tn * nh[i];            // stress-free: tangential traction removed (G17)
-  T qn = v.q[0] * nh[0] + v.q[1] * nh[1] + v.q[2] * nh[2];
+  T qn = q[0] * nh[0] + q[1] * nh[1] + q[2] * nh[2];
   if (wall == -1 && (ph.flags & F_QBOT)) qn = -ph.q_bottom;     // Eq. 32: q = q_b r_hat, outward normal = -r_hat
-  T res = T(0);
-  if (bc != 0) {                                                // radial-field wall: resistive terms as computed
-    res = ph.eta * (v.BxJ[0] * nh[0] + v.BxJ[1] * nh[1] + v.BxJ[2] * nh[2]);
-    for (int i = 0; i < 3; ++i)
-      for (int j = 0; j < 3; ++j) F[5 + i] += nh[j] * ph.eta * (v.dB[i][j] - v.dB[j][i]);
+  for (int c = 0; c < 9; ++c) F[c] = T(0);
+  T work = T(0);
+  for (int i = 0; i < 3; ++i) {
+    T ti = tc[i][0] * nh[0] + tc[i][1] * nh[1] + tc[i][2] * nh[2];     // traction of the conditioned stress
+    F[1 + i] = ti;
+    work += w.u[i] * ti;                                               // U_b . t (U_b is tangent, t is normal: round-off)
   }
-  F[4] = T(0) /* U_b . t = 0 */ - qn + res;
+  F[4] = work - qn + ph.eta * (BxJ[0] * nh[0] + BxJ[1] * nh[1] + BxJ[2] * nh[2]);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) F[5 + i] += nh[j] * ph.eta * (dBc[i][j] - dBc[j][i]);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -303,13 +393,15 @@ struct Ops {
   int n;
   std::vector<T> xs, xf;
   std::vector<T> Isf, Dfs, Efs, Dff;
-  explicit Ops(int n_) : n(n_), xs(n_), xf(n_ + 1) {
+  std::vector<T> wq;   // [n] quadrature weights at the solution points: w_i = int_0^1 h_i(X) dX (volume integrals, Eq. 34-35)
+  explicit Ops(int n_) : n(n_), xs(n_), xf(n_ + 1), wq(n_, T(0)) {
     const T pi = std::acos(T(-1));
     for (int k = 1; k <= n; ++k) xs[k - 1] = T(0.5) * (T(1) - std::cos(T(2 * k - 1) * pi / T(2 * n)));   // Eq. 18
     // flux points: 0, roots of the Legendre polynomial P_{n-1} mapped to [0,1], 1  (G1)
     xf[0] = T(0);
     xf[n] = T(1);
     int m = n - 1;
+    std::vector<T> gw(n + 1, T(0));   // weights of the (n-1)-point Gauss-Legendre rule on [0,1] at the interior flux points
     for (int k = 1; k <= m; ++k) {
       T z = -std::cos(pi * (T(k) - T(0.25)) / (T(m) + T(0.5)));          // ascending initial guesses
       for (int it = 0; it < 100; ++it) {
@@ -326,6 +418,17 @@ struct Ops {
         if (std::fabs(dz) < T(4) * std::numeric_limits<T>::epsilon()) break;
       }
       xf[k] = T(0.5) * (T(1) + z);
+      {   // Gauss weight 2 / ((1 - z^2) P_m'(z)^2) on [-1,1], halved for [0,1]
+        T p0 = T(1), p1 = z;
+        for (int l = 2; l <= m; ++l) {
+          T p2 = (T(2 * l - 1) * z * p1 - T(l - 1) * p0) / T(l);
+          p0 = p1;
+          p1 = p2;
+        }
+        T pm = (m == 0) ? T(1) : p1, pm1 = (m == 1) ? T(1) : p0;
+        T dp = T(m) * (z * pm - pm1) / (z * z - T(1));
+        gw[k] = T(1) / ((T(1) - z * z) * dp * dp);
+      }
     }
     int N1 = n + 1;
     Isf.resize(N1 * n);
@@ -341,6 +444,10 @@ struct Ops {
       }
     for (int a = 0; a < N1; ++a)
       for (int m2 = 0; m2 < N1; ++m2) Dff[a * N1 + m2] = lagrange_deriv(xf, m2, xf[a]);   // l'_m(X_f,a)
+    // w_i = int_0^1 h_i: h_i has degree n-1 and the (n-1)-point Gauss rule is exact to degree 2n-3 >= n-1, so the integral is
+    // the Gauss sum of h_i over the interior flux points (n = 2: one point, exact to degree 1)
+    for (int i = 0; i < n; ++i)
+      for (int k = 1; k <= m; ++k) wq[i] += gw[k] * Isf[k * n + i];
   }
 };
 
@@ -392,6 +499,7 @@ struct Solver {
   std::vector<T> jinv;   // [E][3 d][3 p][n3]          (grad xi_d)_p at the solution points
   std::vector<T> xsol;   // [E][3][n3]
   std::vector<T> krfl;   // [E][3 fam][nf]             kappa_r at the flux points (only if kr_scale != 0)
+  std::vector<T> rfl;    // [E][3 fam][nf]             distance of the flux points from the origin (wall frame, kappa_r)
   // state and work arrays
   std::vector<T> Q;      // [9][E][n3]
   bool have_state = false;
@@ -460,6 +568,8 @@ struct Solver {
     xsol.assign((size_t)E * 3 * n3, T(0));
     bool need_kr = (ph.kr_scale != T(0));
     if (need_kr) krfl.assign((size_t)E * 3 * nf, T(0));
+    else krfl.clear();
+    rfl.assign((size_t)E * 3 * nf, T(0));
     const int ng = mesh.ng, ng3 = ng * ng * ng, G3 = N1 * N1 * N1;
     std::vector<T> gn(ng);
     for (int q = 0; q < ng; ++q) gn[q] = T(mesh.gnodes[q]);
@@ -570,7 +680,7 @@ struct Solver {
         tensor_eval(&X[c * G3], Efs, n, Efs, n, Efs, n, &xsol[((size_t)e * 3 + c) * n3]);
         for (int s = 0; s < n3; ++s) xsol[((size_t)e * 3 + c) * n3 + s] += x0[c];
       }
-      if (need_kr) {
+      {
         std::vector<T> xf3(3 * nf);
         for (int d = 0; d < 3; ++d) {
           for (int c = 0; c < 3; ++c)
@@ -579,8 +689,9 @@ struct Solver {
           for (int g = 0; g < nf; ++g) {
             T px = xf3[g] + x0[0], py = xf3[nf + g] + x0[1], pz = xf3[2 * nf + g] + x0[2];
             T r = std::sqrt(px * px + py * py + pz * pz);
+            rfl[((size_t)e * 3 + d) * nf + g] = r;
             T w = r * ph.kr_wscale;
-            krfl[((size_t)e * 3 + d) * nf + g] = ph.kr_scale * (ph.kr_c[0] + ph.kr_c[1] * w + ph.kr_c[2] * w * w);
+            if (need_kr) krfl[((size_t)e * 3 + d) * nf + g] = ph.kr_scale * (ph.kr_c[0] + ph.kr_c[1] * w + ph.kr_c[2] * w * w);
           }
         }
       }
@@ -748,7 +859,7 @@ struct Solver {
                 T Qb[9];
                 wall_state(ph, ne, Qi, nh, Qb);
                 flux_inviscid(ph, Qb, nh, Fc, /*wall=*/true);
-                if (diff) flux_wall_viscous(ph, ne, Qb, Gi, nh, kr, Fv);
+                if (diff) flux_wall_viscous(ph, ne, Qb, Gi, nh, rfl[((size_t)e * 3 + d) * nf + ix], kr, Fv);
                 flux_inviscid_abs(ph, Qb, nh, Fa, /*wall=*/true);
                 for (int v = 0; v < 9; ++v) Fa[v] += std::fabs(Fv[v]);
               }
@@ -798,6 +909,27 @@ struct Solver {
       }
     }
     Q = u[nstages];
+  }
+
+  // Eq. 34-35: V = int dV, KE = (1/V) int 1/2 rho U.U dV, E_B = (1/V) int 1/2 B.B dV, with the
+  // interpolatory quadrature of the solution points: int f dV = sum_e sum_ijk w_i w_j w_k |J| f.  Sums are kept in long double.
+  void diagnostics(double out[3]) const {
+    long double V = 0, KE = 0, EB = 0;
+    for (int64_t e = 0; e < E; ++e)
+      for (int k = 0; k < n; ++k)
+        for (int j = 0; j < n; ++j)
+          for (int i = 0; i < n; ++i) {
+            int s = (k * n + j) * n + i;
+            T Qp[9];
+            for (int v = 0; v < 9; ++v) Qp[v] = Q[((size_t)v * E + e) * n3 + s];
+            long double wJ = (long double)(op.wq[i] * op.wq[j] * op.wq[k]) * (long double)detJ[(size_t)e * n3 + s];
+            V += wJ;
+            KE += wJ * (long double)(T(0.5) * (Qp[1] * Qp[1] + Qp[2] * Qp[2] + Qp[3] * Qp[3]) / Qp[0]);
+            EB += wJ * (long double)(T(0.5) * (Qp[5] * Qp[5] + Qp[6] * Qp[6] + Qp[7] * Qp[7]));
+          }
+    out[0] = (double)V;
+    out[1] = (double)(KE / V);
+    out[2] = (double)(EB / V);
   }
 
   T max_wavespeed() const {
@@ -884,6 +1016,17 @@ int oracle_max_wavespeed(oracle_ctx* c, double* out) {
   *out = c->d ? c->d->max_wavespeed() : (double)c->l->max_wavespeed();
   return 0;
 }
+int oracle_diagnostics(oracle_ctx* c, double* out) {
+  if (!c || !out) return -1;
+  if (c->d) c->d->diagnostics(out); else c->l->diagnostics(out);
+  return 0;
+}
+int oracle_quadrature_weights(int order, double* w) {
+  if (order < 2 || order > 12 || !w) return -1;
+  Ops<long double> o(order);
+  for (int i = 0; i < order; ++i) w[i] = (double)o.wq[i];
+  return 0;
+}
 int oracle_get_gradient(oracle_ctx* c, double* g) {
   if (!c || !g) return -1;
   if (c->d) {
@@ -957,8 +1100,17 @@ void oracle_wall_state(const oracle_physics* p, int wall, const double* Q, const
 void oracle_flux_wall_inviscid(const oracle_physics* p, const double* Qb, const double* nh, double* F) {
   flux_inviscid(Phys<double>(*p), Qb, nh, F, true);
 }
-void oracle_flux_wall_viscous(const oracle_physics* p, int wall, const double* Qb, const double* G, const double* nh, double kr, double* F) {
-  flux_wall_viscous(Phys<double>(*p), wall, Qb, G, nh, kr, F);
+void oracle_flux_wall_viscous(const oracle_physics* p, int wall, const double* Qb, const double* G, const double* nh, double rw,
+                              double kr, double* F) {
+  flux_wall_viscous(Phys<double>(*p), wall, Qb, G, nh, rw, kr, F);
+}
+void oracle_wall_condition_gradB(int bc, const double* dB, const double* Bb, const double* er, double rw, double* dBc) {
+  double a[3][3], c[3][3];
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) a[i][j] = dB[i * 3 + j];
+  wall_condition_gradB<double>(bc, a, Bb, er, rw, c);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) dBc[i * 3 + j] = c[i][j];
 }
 void oracle_source(const oracle_physics* p, const double* Q, const double* G, const double* x, double* M, double* Mabs) {
   source(Phys<double>(*p), Q, G, x, M, Mabs);

@@ -59,6 +59,10 @@ int  oracle_residual(oracle_ctx*, double* r, double* a);
 int  oracle_step(oracle_ctx*, double dt, int nstages);   /* 5: SSPRK(5,3); 3: SSPRK(3,3); 1: Euler */
 int  oracle_max_wavespeed(oracle_ctx*, double* out);
 int  oracle_get_gradient(oracle_ctx*, double* g);        /* BR1 gradient of the current state */
+/* out[3] = V, KE, E_B of the current state (Eq. 34-35) by the solution-point quadrature */
+int  oracle_diagnostics(oracle_ctx*, double* out);
+/* w [n]: interpolatory quadrature weights on the solution points of [0,1], w_i = int h_i (Eq. 19) */
+int  oracle_quadrature_weights(int order, double* w);
 /* any pointer may be NULL. detJ [E][n^3]; S [E][3 fam][3 comp][n^2(n+1)]; xsol [3][E][n^3];
    jinv [E][3 d][3 p][n^3] = (grad xi_d)_p */
 int  oracle_get_geometry(oracle_ctx*, double* detJ, double* S, double* xsol, double* jinv);
@@ -80,8 +84,13 @@ double oracle_wavespeed(const oracle_physics*, const double* Q);
 /* wall = -1 inner / -2 outer */
 void oracle_wall_state(const oracle_physics*, int wall, const double* Q, const double* nhat, double* Qb);
 void oracle_flux_wall_inviscid(const oracle_physics*, const double* Qb, const double* nhat, double* F);
+/* wall viscous flux along nhat from (Q_b, grad Q_in) with the wall conditions applied to the wall gradients:
+   rw = distance of the wall point from the origin (<= 0: plane wall) */
 void oracle_flux_wall_viscous(const oracle_physics*, int wall, const double* Qb, const double* G, const double* nhat,
-                              double kr, double* F);
+                              double rw, double kr, double* F);
+/* the conditioned Jacobian of B at a wall point: dB, dBc [3][3] row-major d_j B_i; bc 0 perfectly conducting, 1 perfectly
+   radial; Bb the wall state's field; er the wall's radial unit vector; rw as above */
+void oracle_wall_condition_gradB(int bc, const double* dB, const double* Bb, const double* er, double rw, double* dBc);
 void oracle_source(const oracle_physics*, const double* Q, const double* G, const double* x, double* M, double* Mabs);
 
 #ifdef __cplusplus

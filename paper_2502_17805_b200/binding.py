@@ -18,7 +18,7 @@ CHORUS_OK, CHORUS_EINVAL, CHORUS_ENOMEM, CHORUS_ECUDA, CHORUS_ESTATE = 0, -1, -2
 
 # every symbol include/chorus.h declares
 SYMBOLS = ("chorus_init", "chorus_free", "chorus_set_physics", "chorus_set_state", "chorus_get_state", "chorus_residual",
-           "chorus_step", "chorus_max_wavespeed", "chorus_last_error", "chorus_get_geometry", "chorus_get_gradient",
+           "chorus_step", "chorus_max_wavespeed", "chorus_diagnostics", "chorus_last_error", "chorus_get_geometry", "chorus_get_gradient",
            "chorus_get_operators", "chorus_launch_count", "chorus_profile", "chorus_profile_read", "chorus_fp64_peak")
 
 
@@ -73,6 +73,7 @@ def lib():
         L.chorus_residual.argtypes = [V, V, I]
         L.chorus_step.argtypes = [V, D, I]
         L.chorus_max_wavespeed.argtypes = [V, C.POINTER(D)]
+        L.chorus_diagnostics.argtypes = [V, V]
         L.chorus_last_error.argtypes = [V]
         L.chorus_last_error.restype = C.c_char_p
         L.chorus_get_geometry.argtypes = [V, V, V, V, V, I]
@@ -197,6 +198,12 @@ class Chorus:
         v = C.c_double()
         self._check(lib().chorus_max_wavespeed(self._ctx, C.byref(v)))
         return v.value
+
+    def diagnostics(self):
+        """dict(V, KE, EB): shell volume, volume-averaged kinetic and magnetic energy (Eq. 34-35)."""
+        out = np.empty(3)
+        self._check(lib().chorus_diagnostics(self._ctx, out.ctypes.data_as(C.c_void_p)))
+        return dict(V=float(out[0]), KE=float(out[1]), EB=float(out[2]))
 
     def gradient(self, device=False):
         out = self._out((27, self.E, self.n ** 3), device)

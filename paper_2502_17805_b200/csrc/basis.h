@@ -19,6 +19,7 @@ struct Basis {
   std::vector<double> Efs;      // [n][(n+1)]    l_m(xs_i)              flux polynomial evaluated at solution points (geometry)
   std::vector<double> Dff;      // [(n+1)][(n+1)] l'_m(xf_a)            derivative on the flux-point grid (geometry)
   std::vector<double> Dss;      // [n][n]        sum_{m interior} Dfs[i][m] Isf[m][l]   (BR1 gradient, interior part)
+  std::vector<double> wq;       // [n]           quadrature weights at the solution points (volume integrals, Eq. 34-35)
 };
 
 namespace detail {
@@ -145,6 +146,15 @@ inline Basis make_basis(int n) {
   B.Efs = cvt(Efs);
   B.Dff = cvt(Dff);
   B.Dss = cvt(Dss);
+  // Interpolatory quadrature on the Chebyshev-Gauss points of [0,1] = Fejer's first rule, closed form:
+  // w_k = (1/n) [1 - 2 sum_{j=1}^{n/2} cos(2 j theta_k) / (4 j^2 - 1)], theta_k = (2k - 1) pi / (2n)
+  B.wq.resize(n);
+  for (int k = 1; k <= n; ++k) {
+    const real th = (2 * k - 1) * pi / (2 * n);
+    real w = 1;
+    for (int q = 1; q <= n / 2; ++q) w -= 2 * cosl(2 * q * th) / (4.0L * q * q - 1);
+    B.wq[k - 1] = (double)(w / n);
+  }
   return B;
 }
 

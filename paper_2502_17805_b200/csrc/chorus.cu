@@ -5,6 +5,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -46,6 +47,7 @@ struct chorus_ctx {
   bool traces_valid = false;              // ... if any does
   double* d_Vf = nullptr;
   unsigned long long* d_ws = nullptr;
+  double *d_wq = nullptr, *d_diag = nullptr;   // quadrature weights [n]; diagnostics partial sums [kDiagBlocks + 1][3]
   unsigned* d_arrivals = nullptr;   // per-SM CTA arrival counters of the main kernel
   double* d_scratch = nullptr;      // per-CTA global scratch of the scalar kernels' SPILL variants (orders 8, 9 with diffusion)
   size_t scratch_doubles = 0;
@@ -58,6 +60,8 @@ struct chorus_ctx {
 };
 
 namespace {
+
+constexpr int kDiagBlocks = 1184;   // 8 x 148: blocks of the diagnostics reduction (fixed, so the summation tree is too)
 
 int fail(chorus_ctx* c, int code, const std::string& msg) {
   if (c) c->err = msg;
@@ -410,6 +414,7 @@ int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chor
   if ((rc = upload(c, &c->d_Dff, B.Dff.data(), B.Dff.size()))) return bail(rc);
   if ((rc = upload(c, &c->d_Efs, B.Efs.data(), B.Efs.size()))) return bail(rc);
   if ((rc = upload(c, &c->d_Dfs, B.Dfs.data(), B.Dfs.size()))) return bail(rc);
+  if ((rc = upload(c, &c->d_wq, B.wq.data(), B.wq.size()))) return bail(rc);
   if ((rc = upload(c, &c->d_xyz, mesh->xyz, (size_t)c->E * 3 * ng3))) return bail(rc);
   if ((rc = upload(c, &c->d_nbr_elem, mesh->nbr_elem, (size_t)c->E * 6))) return bail(rc);
   if ((rc = upload(c, &c->d_nbr_face, mesh->nbr_face, (size_t)c->E * 6))) return bail(rc);
@@ -421,6 +426,7 @@ int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chor
             dalloc(&c->d_Vf, E * 42 * c->n2);
   for (int k = 0; k < 5 && ok; ++k) ok = dalloc(&c->d_U[k], E * 9 * c->n3);
   ok = ok && cudaMalloc(&c->d_ws, sizeof(unsigned long long)) == cudaSuccess;
+  ok = ok && dalloc(&c->d_diag, (size_t)(kDiagBlocks + 1) * 3);
   ok = ok && cudaMalloc(&c->d_arrivals, sizeof(unsigned) * 1024) == cudaSuccess &&
        cudaMemsetAsync(c->d_arrivals, 0, sizeof(unsigned) * 1024, c->stream) == cudaSuccess;
   if (!ok) return bail(CHORUS_ENOMEM);
@@ -438,7 +444,7 @@ void chorus_free(chorus_ctx* c) {
   cudaFree(c->d_Gm); cudaFree(c->d_Dff); cudaFree(c->d_Efs); cudaFree(c->d_Dfs);
   cudaFree(c->d_Sfl); cudaFree(c->d_detJ); cudaFree(c->d_jinv); cudaFree(c->d_xsol); cudaFree(c->d_krfl); cudaFree(c->d_nfc);
   for (int k = 0; k < 5; ++k) cudaFree(c->d_U[k]);
-  cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_ws); cudaFree(c->d_arrivals); cudaFree(c->d_scratch);
+  cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_ws); cudaFree(c->d_wq); cudaFree(c->d_diag); cudaFree(c->d_arrivals); cudaFree(c->d_scratch);
   for (auto& v : c->prof_ev)
     for (auto& ev : v) {
       cudaEventDestroy(ev.first);
@@ -579,6 +585,22 @@ int chorus_max_wavespeed(chorus_ctx* c, double* out) {
   std::memcpy(&v, &bits, sizeof v);
   *out = v;
   if (!std::isfinite(v)) return fail(c, CHORUS_ESTATE, "non-finite wave speed");
+  return CHORUS_OK;
+}
+
+int chorus_diagnostics(chorus_ctx* c, double* out) {
+  if (!c || !out) return CHORUS_EINVAL;
+  if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
+  const int64_t total = c->E * c->n3;
+  const int grid = (int)std::min<int64_t>(kDiagBlocks, (total + 255) / 256);
+  diagnostics_kernel<<<grid, 256, 0, c->stream>>>(c->E, c->n, c->d_wq, c->d_detJ, c->d_U[c->cur], c->d_diag);
+  ++c->launches;
+  CU(c, cudaGetLastError());
+  diagnostics_final_kernel<<<1, 256, 0, c->stream>>>(grid, c->d_diag, c->d_diag + (size_t)kDiagBlocks * 3);
+  ++c->launches;
+  CU(c, cudaGetLastError());
+  CU(c, cudaMemcpyAsync(out, c->d_diag + (size_t)kDiagBlocks * 3, sizeof(double) * 3, cudaMemcpyDeviceToHost, c->stream));
+  CU(c, cudaStreamSynchronize(c->stream));
   return CHORUS_OK;
 }
 

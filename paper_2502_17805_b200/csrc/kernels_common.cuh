@@ -164,4 +164,54 @@ __global__ void __launch_bounds__(256) wavespeed_kernel(int64_t E, int n3, PhysD
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Volume integrals of Eq. 34-35 by the solution-point quadrature  int f dV = sum w_i w_j w_k |J| f:
+// sum |J| w, sum |J| w 1/2 rho U.U, sum |J| w 1/2 B.B.  Deterministic: one partial per block (warp shuffle tree, then the
+// block's warps in order), then one block adds the partials in a fixed tree -- no atomics, bit-reproducible.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void block_sum3(double& a, double& b, double& c, double (*sh)[3]) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    a += __shfl_xor_sync(0xffffffffu, a, o);
+    b += __shfl_xor_sync(0xffffffffu, b, o);
+    c += __shfl_xor_sync(0xffffffffu, c, o);
+  }
+  const int warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) { sh[warp][0] = a; sh[warp][1] = b; sh[warp][2] = c; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    a = sh[0][0]; b = sh[0][1]; c = sh[0][2];
+    for (int w = 1; w < nw; ++w) { a += sh[w][0]; b += sh[w][1]; c += sh[w][2]; }
+  }
+}
+__global__ void __launch_bounds__(256) diagnostics_kernel(int64_t E, int n, const double* __restrict__ wq, const double* __restrict__ detJ,
+                                                         const double* __restrict__ Qe, double* __restrict__ partial /*[grid][3]*/) {
+  __shared__ double sh[8][3];
+  const int n3 = n * n * n;
+  double V = 0.0, KE = 0.0, EB = 0.0;
+  const int64_t total = E * n3;
+  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t e = t / n3;
+    const int s = (int)(t % n3);
+    const int i = s % n, j = (s / n) % n, k = s / (n * n);
+    const double wJ = wq[i] * wq[j] * wq[k] * detJ[t];
+    const double* q = Qe + e * 9 * n3 + s;
+    const double rho = q[0], m1 = q[n3], m2 = q[2 * n3], m3 = q[3 * n3];
+    const double b1 = q[5 * n3], b2 = q[6 * n3], b3 = q[7 * n3];
+    V += wJ;
+    KE += wJ * (0.5 * (m1 * m1 + m2 * m2 + m3 * m3) / rho);
+    EB += wJ * (0.5 * (b1 * b1 + b2 * b2 + b3 * b3));
+  }
+  block_sum3(V, KE, EB, sh);
+  if (threadIdx.x == 0) { partial[blockIdx.x * 3 + 0] = V; partial[blockIdx.x * 3 + 1] = KE; partial[blockIdx.x * 3 + 2] = EB; }
+}
+__global__ void __launch_bounds__(256) diagnostics_final_kernel(int nparts, const double* __restrict__ partial, double* __restrict__ out /*[3]*/) {
+  __shared__ double sh[8][3];
+  double V = 0.0, KE = 0.0, EB = 0.0;
+  for (int t = threadIdx.x; t < nparts; t += blockDim.x) { V += partial[t * 3]; KE += partial[t * 3 + 1]; EB += partial[t * 3 + 2]; }
+  block_sum3(V, KE, EB, sh);
+  if (threadIdx.x == 0) { out[0] = V; out[1] = KE / V; out[2] = EB / V; }
+}
+
 }  // namespace chorus

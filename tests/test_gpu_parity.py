@@ -111,14 +111,27 @@ def test_nonequilibrium_input_naive_relative_error():
 
 
 @pytest.mark.parametrize("wall_opts", [dict(bc_mag_inner=I.BC_RADIAL, bc_mag_outer=I.BC_CONDUCTING),
+                                       dict(bc_mag_inner=I.BC_CONDUCTING, bc_mag_outer=I.BC_CONDUCTING),
+                                       dict(bc_mag_inner=I.BC_RADIAL, bc_mag_outer=I.BC_RADIAL, T_top=0.05, q_bottom=0.02,
+                                            extra_flags=I.FLAG_FIXED_T_OUTER | I.FLAG_FIXED_FLUX_INNER),
+                                       dict(bc_mag_inner=I.BC_CONDUCTING, bc_mag_outer=I.BC_RADIAL, kr_scale=2e-3, kr_c=(1.0, -0.5, 0.25),
+                                            T_top=0.05, q_bottom=0.02, extra_flags=I.FLAG_FIXED_T_OUTER | I.FLAG_FIXED_FLUX_INNER),
                                        dict(T_top=0.05, q_bottom=0.02, extra_flags=I.FLAG_FIXED_T_OUTER | I.FLAG_FIXED_FLUX_INNER),
                                        dict(extra_flags=I.FLAG_CENTRIFUGAL),
                                        dict(kr_scale=2e-3, kr_c=(1.0, -0.5, 0.25), kr_wscale=1.3)])
 def test_wall_and_option_variants_parity(wall_opts):
     kw = dict(wall_opts)
     extra = kw.pop("extra_flags", 0)
+    """Both magnetic wall types on each wall, thermal wall options, centrifugal term, kappa_r(r).  The oracle applies the wall
+    conditions to the wall gradients literally (Jacobian of B and stress tensor in the spherical frame of the wall point,
+    PAPER.md:198, reading G29); the kernels use the closed form those conditions reduce to (DESIGN.md 2)."""
     w, mesh, o, g, Q, phys = shell_case(5, 3, 2, 3.0, 7, 2e-3, u_amp=0.01, b_amp=0.05, extra_flags=extra, **kw)
     check_residual(o, g)
+    _, xf, _, _ = P.get_operators(5)
+    dt = w.dt(o.max_wavespeed(), xf[1] - xf[0])
+    for _ in range(2):
+        o.step(dt, 5); g.step(dt, 5)
+    assert g25_error(g.get_state(), o.get_state(), phys.c_h).max() <= STATE_TOL
 
 
 def test_all_orientation_codes_parity():
@@ -250,3 +263,56 @@ def test_bitwise_reproducible_across_launches(n, diff):
         finals.append(g.get_state())
     np.testing.assert_array_equal(finals[0], finals[1])
     np.testing.assert_array_equal(finals[0], finals[2])
+
+
+def test_diagnostics_parity_and_reproducibility():
+    """chorus_diagnostics (V, KE of Eq. 34, E_B of Eq. 35) against the oracle's literal long-double sums, on a small and on a
+    768-element shell, before and after a step; the tree reduction has no atomics: bit-identical from call to call."""
+    for nz, nr, n in ((4, 2, 6), (8, 2, 5)):
+        w, mesh, o, g, Q, phys = shell_case(n, nz, nr, 3.0, 21, 1e-3, u_amp=0.05, b_amp=0.2)
+        for it in range(2):
+            d, d_ref = g.diagnostics(), o.diagnostics()
+            for k in ("V", "KE", "EB"):
+                assert abs(d[k] / d_ref[k] - 1) <= 1e-13, (k, d[k], d_ref[k])
+            assert g.diagnostics() == d
+            _, xf, _, _ = P.get_operators(n)
+            dt = w.dt(o.max_wavespeed(), xf[1] - xf[0])
+            o.step(dt, 5); g.step(dt, 5)
+    g2 = P.Chorus(mesh, n, phys)
+    with pytest.raises(P.ChorusError) as ei:
+        g2.diagnostics()
+    assert ei.value.code == -4
+
+
+@pytest.mark.parametrize("obl", [0.1, 0.3])
+def test_oblate_shell_geometry_and_residual_parity(obl):
+    """Oblate shells through the generic geometry-node input: metrics, residual with all terms, two steps."""
+    n = 6
+    sh = I.Shell(N_rho=3.0)
+    w = I.Workload("oblate", n, 4, 2, 3.0, 13, 1e-3, True, shell=sh)
+    mesh = I.cubed_sphere_shell(4, 2, sh.r_b, sh.r_t, I.lobatto_abscissae(n + 1), oblateness=obl)
+    o = ob.Oracle(mesh, n, I.Physics())
+    go = o.geometry()
+    Q = I.shell_state(go["xsol"], sh, 13, u_amp=0.01, b_amp=0.05)
+    o.set_state(Q)
+    phys = w.physics(o.max_wavespeed())
+    o.set_physics(phys)
+    g = P.Chorus(mesh, n, phys)
+    gg = g.geometry()
+    for k in ("detJ", "S", "xsol", "jinv"):
+        assert np.abs(gg[k] - go[k]).max() <= GEO_TOL * np.abs(go[k]).max(), k
+    g.set_state(Q)
+    check_residual(o, g)
+    _, xf, _, _ = P.get_operators(n)
+    dt = w.dt(o.max_wavespeed(), xf[1] - xf[0])
+    for _ in range(2):
+        o.step(dt, 5); g.step(dt, 5)
+    assert g25_error(g.get_state(), o.get_state(), phys.c_h).max() <= STATE_TOL
+    # free stream on the GPU: a uniform static state is preserved to round-off on the oblate mesh
+    g.set_physics(phys.copy(flags=I.FLAG_DIFFUSION))
+    o.set_physics(phys.copy(flags=I.FLAG_DIFFUSION))
+    U = np.empty_like(Q)
+    U[:] = I.conserved(1.2, np.zeros(3), 1.5, np.zeros(3), np.float64(0.0), 5 / 3)[:, None, None]
+    g.set_state(U); o.set_state(U)
+    _, a = o.residual(True)
+    assert np.abs(g.residual()).max() <= 1e-12 * a.max()

@@ -184,3 +184,75 @@ def test_p3_freestream_through_every_orientation_code():
     o.set_state(Q)
     r, a = o.residual(True)
     assert np.abs(r).max() <= 1e-13 * a.max()
+
+
+# ------------------------------------------------------------------------------- oblate shells
+@pytest.mark.parametrize("n,obl", [(6, 0.1), (4, 0.25)])
+def test_p3_oblate_shell_freestream_and_volume(n, obl):
+    """"It is also possible to generate oblate meshes": the z axis of the shell scaled by 1 - e.  The map is no
+    longer radial, so nothing of the spherical closed form of the metrics survives -- but the curl-form metrics still preserve
+    a free stream to round-off, the mesh stays right-handed, and the volume is exactly (1 - e) times the spherical one."""
+    nz, nr = 4, 3
+    m = I.cubed_sphere_shell(nz, nr, RB, RT, I.lobatto_abscissae(n + 1), oblateness=obl)
+    ms = I.cubed_sphere_shell(nz, nr, RB, RT, I.lobatto_abscissae(n + 1))
+    np.testing.assert_array_equal(m["nbr_elem"], ms["nbr_elem"])          # same topology
+    np.testing.assert_allclose(m["xyz"][:, 2], (1 - obl) * ms["xyz"][:, 2], rtol=1e-15)
+    o = ob.Oracle(m, n, I.Physics(c_h=1.0, flags=0))
+    geo, geo_s = o.geometry(), ob.Oracle(ms, n, I.Physics()).geometry()
+    assert geo["detJ"].min() > 0
+    E = m["n_elem"]
+    Q = np.zeros((9, E, n ** 3))
+    Q[:] = I.conserved(1.0, np.array([0.3, -0.2, 0.1]), 1.5, np.array([0.5, 0.25, -0.4]), np.float64(0.1), 5 / 3)[:, None, None]
+    o.set_state(Q)
+    r, a = o.residual(True)
+    mid = (np.arange(E) // (nz * nz)) % nr == 1                 # elements not touching a wall
+    assert np.abs(r[:, mid]).max() <= 1e-12 * a[:, mid].max()
+    assert np.abs(o.gradient()[:, mid]).max() < 1e-11
+    # |J| = (1 - e) |J|_sphere point by point (the map is the spherical one followed by a linear stretch), hence the volume
+    np.testing.assert_allclose(geo["detJ"], (1 - obl) * geo_s["detJ"], rtol=1e-11)
+    vol = (geo["detJ"] * w3(n)[None, :]).sum()
+    assert abs(vol / ((1 - obl) * 4 * np.pi / 3 * (RT ** 3 - RB ** 3)) - 1) < (1e-8 if n == 6 else 1e-5)
+    # the area vectors transform with the cofactor of diag(1, 1, 1 - e): (S_x, S_y, S_z) = ((1-e) S_x, (1-e) S_y, S_z)_sphere
+    np.testing.assert_allclose(geo["S"][:, :, 0], (1 - obl) * geo_s["S"][:, :, 0], rtol=0, atol=1e-12 * np.abs(geo_s["S"]).max())
+    np.testing.assert_allclose(geo["S"][:, :, 2], geo_s["S"][:, :, 2], rtol=0, atol=1e-12 * np.abs(geo_s["S"]).max())
+
+
+# ------------------------------------------------------------------------------- volume integrals (Eq. 34-35)
+def test_quadrature_weights_closed_form_exactness_and_telescoping():
+    """w_i = int_0^1 h_i (the oracle integrates the Lagrange basis of Eq. 19 with a Gauss rule): equal to Fejer's first rule in
+    closed form, exact for x^k, k <= n-1, and sum_i w_i l'_m(X_s,i) = delta_{m,n} - delta_{m,0} (the telescoping
+    identity behind mass conservation, pin P12)."""
+    for n in range(2, 10):
+        w = ob.quadrature_weights(n)
+        np.testing.assert_allclose(w, fejer1_weights(n), rtol=0, atol=2e-16)
+        xs, _ = ob.nodes(n)
+        for k in range(n):
+            assert abs(w @ xs ** k - 1.0 / (k + 1)) < 1e-15
+        assert abs(w @ xs ** (n + 1) - 1.0 / (n + 2)) > 1e-9 or n % 2 == 1     # and not beyond its degree (symmetric rules gain one)
+        _, Dfs, _, _ = ob.operators(n)
+        tel = w @ Dfs
+        ref = np.zeros(n + 1); ref[0], ref[n] = -1.0, 1.0
+        np.testing.assert_allclose(tel, ref, rtol=0, atol=1e-13)
+
+
+def test_diagnostics_closed_forms_on_the_shell():
+    """KE and E_B of Eq. 34-35 for fields with closed forms on the spherical shell: rigid rotation of a uniform-density fluid,
+    int (x^2 + y^2) dV = (2/3) 4 pi (r_t^5 - r_b^5)/5; a uniform field (E_B = |B|^2/2 exactly, whatever V); |B| = r."""
+    n, nz, nr = 6, 4, 2
+    m = I.cubed_sphere_shell(nz, nr, RB, RT, I.lobatto_abscissae(n + 1))
+    o = ob.Oracle(m, n, I.Physics())
+    x = o.geometry()["xsol"]
+    V_ref = 4 * np.pi / 3 * (RT ** 3 - RB ** 3)
+    I5 = 4 * np.pi * (RT ** 5 - RB ** 5) / 5                    # int r^2 dV
+    rho0, Om = 1.7, 0.4
+    one = np.ones_like(x[0])
+    U = np.stack([-Om * x[1], Om * x[0], 0 * one])
+    B0 = np.array([0.3, -0.2, 0.5])
+    o.set_state(I.conserved(rho0 * one, U, one, B0[:, None, None] * one, 0 * one, 5 / 3))
+    d = o.diagnostics()
+    assert abs(d["V"] / V_ref - 1) < 1e-8
+    assert abs(d["KE"] / (0.5 * rho0 * Om ** 2 * (2 / 3) * I5 / V_ref) - 1) < 1e-7
+    assert abs(d["EB"] / (0.5 * B0 @ B0) - 1) < 1e-14
+    o.set_state(I.conserved(rho0 * one, 0 * U, one, x, 0 * one, 5 / 3))           # B = x, |B| = r
+    d = o.diagnostics()
+    assert d["KE"] == 0.0 and abs(d["EB"] / (0.5 * I5 / V_ref) - 1) < 1e-7

@@ -195,7 +195,7 @@ def test_wall_state_and_fluxes(wall, bc):
     Fv = ob.flux_wall_viscous(ph, wall, Qb, G, nh)
     np.testing.assert_allclose(np.cross(Fv[1:4], nh), 0.0, atol=1e-15)
     if bc == I.BC_CONDUCTING:
-        np.testing.assert_allclose(Fv[5:8], 0.0, atol=0)
+        np.testing.assert_allclose(Fv[5:8], 0.0, atol=1e-14 * np.abs(G).max())   # J = J_r r_hat: no resistive flux through the wall
     gen = ob.flux_viscous(ph, Qb, G, nh)
     np.testing.assert_allclose(Fv[1:4] @ nh, gen[1:4] @ nh, atol=1e-13)      # normal traction kept
 
@@ -212,6 +212,94 @@ def test_wall_thermal_options():
     G = np.zeros(27)
     Fv = ob.flux_wall_viscous(ph, -1, Qi, G, nh)
     assert abs(Fv[4] - 0.37) < 1e-15                                 # -q.n with q.n = -q_bottom (Eq. 32)
+
+
+def _rot(rng):
+    A = rng.normal(size=(3, 3))
+    Qm, _ = np.linalg.qr(A)
+    return Qm * np.sign(np.linalg.det(Qm))
+
+
+def test_wall_gradient_conditions_on_the_jacobian_of_B():
+    """conductor B_r = d_r(r B_theta) = d_r(r B_phi) = 0; radial B_theta = B_phi = 0, d_r(r^2 B_r) = 0, imposed on
+    the Jacobian of B in the spherical frame of the wall point (reading G29).  Fields that satisfy a condition exactly keep their
+    Jacobian; a generic Jacobian loses its tangential current (conductor) or its radial current and its divergence (radial);
+    the operation is covariant (independent of the tangent vectors chosen for the frame)."""
+    rng = np.random.default_rng(11)
+    x = np.array([0.31, -0.52, 0.44]); r = np.linalg.norm(x); er = x / r
+    eye = np.eye(3)
+    # perfectly radial field B = x/r^3 (B_r = 1/r^2): d_j B_i = delta_ij/r^3 - 3 x_i x_j/r^5
+    B = x / r ** 3
+    dB = eye / r ** 3 - 3 * np.outer(x, x) / r ** 5
+    np.testing.assert_allclose(ob.wall_condition_gradB(I.BC_RADIAL, dB, B, er, r), dB, atol=1e-14 * np.abs(dB).max())
+    # toroidal field B = (z_hat x x)/r^2 = sin(theta) phi_hat / r: B_r = 0, r B_phi independent of r
+    A = np.array([-x[1], x[0], 0.0])
+    dA = np.array([[0.0, -1.0, 0.0], [1.0, 0.0, 0.0], [0.0, 0.0, 0.0]])
+    B = A / r ** 2
+    dB = dA / r ** 2 - 2 * np.outer(A, x) / r ** 4
+    assert abs(B @ er) < 1e-16
+    np.testing.assert_allclose(ob.wall_condition_gradB(I.BC_CONDUCTING, dB, B, er, r), dB, atol=1e-14 * np.abs(dB).max())
+    assert np.abs(ob.wall_condition_gradB(I.BC_RADIAL, dB, 0 * B, er, r) - dB).max() > 0.1 * np.abs(dB).max()   # ... and is not a radial-wall field
+    # generic Jacobians
+    curl = lambda D: np.array([D[2, 1] - D[1, 2], D[0, 2] - D[2, 0], D[1, 0] - D[0, 1]])
+    for _ in range(20):
+        dB = rng.normal(size=(3, 3)); Bf = rng.normal(size=3); er = unit(rng.normal(size=3)); rw = rng.uniform(0.5, 2.0)
+        Bt, Br = Bf - (Bf @ er) * er, (Bf @ er) * er
+        Dc = ob.wall_condition_gradB(I.BC_CONDUCTING, dB, Bt, er, rw)
+        Jc = curl(Dc)
+        np.testing.assert_allclose(np.cross(Jc, er), 0.0, atol=1e-14)                  # J = J_r r_hat
+        assert abs(Jc @ er - curl(dB) @ er) < 1e-14                                    # ... with J_r as computed
+        assert abs(er @ Dc @ er - er @ dB @ er) < 1e-14                                # d_r B_r is not constrained
+        Dr = ob.wall_condition_gradB(I.BC_RADIAL, dB, Br, er, rw)
+        Jr = curl(Dr)
+        assert abs(np.trace(Dr)) < 1e-14                                               # div B = 0 at the wall
+        assert abs(Jr @ er) < 1e-14                                                    # no radial current
+        np.testing.assert_allclose(np.cross(Jr, er), np.cross(curl(dB), er), atol=1e-14)   # tangential current as computed
+        assert abs(er @ Dr @ er + 2 * (Bf @ er) / rw) < 1e-14                          # d_r(r^2 B_r) = 0
+        Rm = _rot(rng)                                                                 # covariance
+        for bc, Bw in ((I.BC_CONDUCTING, Bt), (I.BC_RADIAL, Br)):
+            D0 = ob.wall_condition_gradB(bc, dB, Bw, er, rw)
+            D1 = ob.wall_condition_gradB(bc, Rm @ dB @ Rm.T, Rm @ Bw, Rm @ er, rw)
+            np.testing.assert_allclose(D1, Rm @ D0 @ Rm.T, atol=1e-14)
+
+
+@pytest.mark.parametrize("wall,bc", [(-1, I.BC_CONDUCTING), (-1, I.BC_RADIAL), (-2, I.BC_CONDUCTING), (-2, I.BC_RADIAL)])
+@pytest.mark.parametrize("thermal", [0, I.FLAG_FIXED_T_OUTER | I.FLAG_FIXED_FLUX_INNER])
+def test_wall_viscous_flux_with_conditioned_gradients_closed_form(wall, bc, thermal):
+    """The wall viscous flux built from the conditioned wall gradients equals, term by term, the closed form the conditions
+    imply: traction (n.tau.n) n with tau of Eq. 8, no viscous work, heat flux -q.n with q of Eq. 9 (or q_bottom, Eq. 32), no
+    resistive flux through a perfect conductor, -eta n x J for a radial-field wall and no Poynting flux in either case; and it
+    does not depend on the radius of the wall (the curvature terms only enter components that carry no flux)."""
+    rng = np.random.default_rng(100 + 7 * wall + bc)
+    ph = PH.copy(bc_mag_inner=bc, bc_mag_outer=bc, T_top=0.9, q_bottom=0.37, flags=I.FLAG_DIFFUSION | thermal)
+    for _ in range(5):
+        Q, _ = rand_state()
+        nh = unit(rng.normal(size=3))
+        Qb = ob.wall_state(ph, wall, Q, nh)
+        rho, ub, Bb, psi = Qb[0], Qb[1:4] / Qb[0], Qb[5:8], Qb[8]
+        pb = (GAM - 1) * (Qb[4] - 0.5 * rho * ub @ ub - 0.5 * Bb @ Bb - 0.5 * psi ** 2)
+        G = rng.normal(size=27)
+        kr = 0.013
+        Fv = ob.flux_wall_viscous(ph, wall, Qb, G, nh, kr=kr, rw=0.83)
+        g = G.reshape(9, 3)
+        du = (g[1:4] - np.outer(ub, g[0])) / rho                                       # d_j u_i
+        tau = rho * ph.nu * (du + du.T) - (2 / 3) * rho * ph.nu * np.trace(du) * np.eye(3)   # Eq. 8, mu = rho nu, Stokes
+        dp = (GAM - 1) * (g[4] - ub @ g[1:4] + 0.5 * (ub @ ub) * g[0] - Bb @ g[5:8] - psi * g[8])
+        dT = (dp - pb / rho * g[0]) / (rho * ph.R_gas)
+        dS = ph.Cp * (dp / (GAM * pb) - g[0] / rho)
+        q = -ph.kappa * rho * (pb / (rho * ph.R_gas)) * dS - kr * rho * ph.Cp * dT     # Eq. 9
+        qn = q @ nh
+        if wall == -1 and thermal:
+            qn = -0.37
+        ref = np.zeros(9)
+        ref[1:4] = (nh @ tau @ nh) * nh
+        ref[4] = -qn
+        J = np.array([g[7, 1] - g[6, 2], g[5, 2] - g[7, 0], g[6, 0] - g[5, 1]])
+        if bc == I.BC_RADIAL:
+            ref[5:8] = -ph.eta * np.cross(nh, J)
+        np.testing.assert_allclose(Fv, ref, atol=2e-13 * max(1.0, np.abs(ref).max()))
+        for rw in (0.0, 0.3, 5.0):
+            np.testing.assert_allclose(ob.flux_wall_viscous(ph, wall, Qb, G, nh, kr=kr, rw=rw), Fv, atol=1e-13 * max(1.0, np.abs(ref).max()))
 
 
 def test_source_terms():

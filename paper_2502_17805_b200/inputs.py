@@ -289,6 +289,57 @@ class Shell:
         return rho, p, T
 
 
+def flux_balanced_profile(shell: "Shell", L: float, kappa: float, kr=None, n_grid: int = 4001):
+    """The "almost flux-balanced" initial stratification of PAPER.md:169-186 (SV, Eq. 28-31), radial profiles on a uniform grid.
+
+    1. polytrope of Eq. 26-27: rho0(r), T0(r), dT0/dr = -g/Cp;
+    2. entropy gradient that carries the luminosity L through every radial layer (Eq. 28 with q_r = L/(4 pi r^2), "the total
+       heat flux from the shell is constant through each radial layer"), on the polytrope's rho0, T0 (Eq. 29):
+           dS/dr = -(L/(4 pi r^2) + kr(r) rho0 Cp dT0/dr) / (kappa rho0 T0)
+       (Eq. 29 as printed lacks the minus sign that its own derivation from Eq. 28 gives: reading G30 of DESIGN.md);
+    3. S(r) = S_b + int_{r_b}^{r} dS/dr (Eq. 30), S_b = Cp ln(p_b^{1/gamma}/rho_b) (Eq. 10), by Simpson's rule;
+    4. new density from hydrostatic balance dp/dr = -rho g (Eq. 25) with p = rho^gamma exp(gamma S/Cp) (Eq. 10 inverted):
+           d rho/dr = -(rho/Cp dS/dr + (g/gamma) rho^(2-gamma) exp(-gamma S/Cp))          (Eq. 31; the printed exponent has
+       the opposite sign, which contradicts Eq. 10 and 25: reading G31), integrated from rho(r_b) = rho_b by classical RK4;
+    5. p = rho^gamma exp(gamma S/Cp), T = p/(rho R).
+    kr: None, or a function r -> kappa_r(r).  Returns dict(r, rho, p, T, S, dSdr) of n_grid points.
+    With L = 0 and kr = None the result is the polytrope itself (isentropic)."""
+    if n_grid < 3 or n_grid % 2 == 0:
+        raise ValueError("n_grid must be odd and >= 3")
+    g_, Cp, gam, R = shell.GM, shell.Cp, shell.gamma, shell.R_gas
+    krf = (lambda r: 0.0 * r) if kr is None else kr
+
+    def dSdr(r):
+        rho0, _, T0 = shell.profile(r)
+        dT0 = -g_ / (Cp * r * r)
+        return -(L / (4.0 * np.pi * r * r) + krf(r) * rho0 * Cp * dT0) / (kappa * rho0 * T0)
+
+    r = np.linspace(shell.r_b, shell.r_t, n_grid)
+    h = r[1] - r[0]
+    rm = 0.5 * (r[:-1] + r[1:])                       # interval mid points
+    f, fm = dSdr(r), dSdr(rm)
+    rho_b, p_b, _ = shell.profile(shell.r_b)
+    S_b = Cp * np.log(p_b ** (1.0 / gam) / rho_b)
+    S = S_b + np.concatenate([[0.0], np.cumsum(h / 6.0 * (f[:-1] + 4.0 * fm + f[1:]))])       # Simpson on every interval
+    # S at the mid points (for RK4): Simpson on the half interval with the quarter point
+    rq = 0.5 * (r[:-1] + rm)
+    Sm = S[:-1] + 0.5 * h / 6.0 * (f[:-1] + 4.0 * dSdr(rq) + fm)
+
+    def rhs(rr, rho, Sv, dS):
+        return -(rho / Cp * dS + (g_ / (rr * rr)) / gam * rho ** (2.0 - gam) * np.exp(-gam * Sv / Cp))
+
+    rho = np.empty(n_grid)
+    rho[0] = rho_b
+    for k in range(n_grid - 1):
+        k1 = rhs(r[k], rho[k], S[k], f[k])
+        k2 = rhs(rm[k], rho[k] + 0.5 * h * k1, Sm[k], fm[k])
+        k3 = rhs(rm[k], rho[k] + 0.5 * h * k2, Sm[k], fm[k])
+        k4 = rhs(r[k + 1], rho[k] + h * k3, S[k + 1], f[k + 1])
+        rho[k + 1] = rho[k] + h / 6.0 * (k1 + 2.0 * k2 + 2.0 * k3 + k4)
+    pr = rho ** gam * np.exp(gam * S / Cp)
+    return dict(r=r, rho=rho, p=pr, T=pr / (rho * R), S=S, dSdr=f)
+
+
 def conserved(rho, U, p, B, psi, gamma):
     """Q = (rho, rho U, E, B, psi) with E of Eq. 3.  U, B: [3,...]."""
     E = p / (gamma - 1.0) + 0.5 * rho * (U ** 2).sum(0) + 0.5 * (B ** 2).sum(0) + 0.5 * psi ** 2
@@ -296,7 +347,7 @@ def conserved(rho, U, p, B, psi, gamma):
 
 
 def shell_state(x_sol: np.ndarray, shell: Shell, seed: int, u_amp: float = 1e-4, b_amp: float = 1e-3,
-                dipole: bool = True, b_random: float = 0.1, flatten: float = 0.0) -> np.ndarray:
+                dipole: bool = True, b_random: float = 0.1, flatten: float = 0.0, background: dict | None = None) -> np.ndarray:
     """Seeded stratified-shell state at the solution-point coordinates x_sol [3,E,n^3].
 
     Recipe (BASELINE.json configs): polytrope of Eq. 26-27; velocity
@@ -304,7 +355,8 @@ def shell_state(x_sol: np.ndarray, shell: Shell, seed: int, u_amp: float = 1e-4,
     B0 = b_amp*sqrt(gamma p_top) ("equipartition" read as B^2 = rho c_s^2 at the top) --
     or B0*uniform(-1,1)^3 alone when dipole=False ("weak random B seed"); psi = 0.
     `flatten` in [0,1] blends the background towards its shell-mean (non-equilibrium inputs
-    for the naive-relative-error parity check).
+    for the naive-relative-error parity check).  `background`: the flux-balanced
+    stratification of Eq. 28-31 (flux_balanced_profile) in place of the polytrope.
     Draw order: pu = uniform(-1,1,(3,E,n^3)) then pb = uniform(-1,1,(3,E,n^3)).
     """
     rng = np.random.Generator(np.random.PCG64(seed))
@@ -312,7 +364,11 @@ def shell_state(x_sol: np.ndarray, shell: Shell, seed: int, u_amp: float = 1e-4,
     pu = rng.uniform(-1.0, 1.0, (3,) + shp)
     pb = rng.uniform(-1.0, 1.0, (3,) + shp)
     r = np.sqrt((x_sol ** 2).sum(0))
-    rho, p, _ = shell.profile(r)
+    if background is not None:      # radial profiles of flux_balanced_profile (Eq. 28-31) instead of the polytrope of Eq. 26
+        rho = np.exp(np.interp(r, background["r"], np.log(background["rho"])))
+        p = np.exp(np.interp(r, background["r"], np.log(background["p"])))
+    else:
+        rho, p, _ = shell.profile(r)
     if flatten:
         rho = (1 - flatten) * rho + flatten * rho.mean()
         p = (1 - flatten) * p + flatten * p.mean()

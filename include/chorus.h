@@ -92,6 +92,36 @@ int chorus_residual(chorus_ctx* ctx, double* r, int on_device);
  * (test aids).  Each stage is a residual evaluation fused with its Runge-Kutta combination. */
 int chorus_step(chorus_ctx* ctx, double dt, int nstages);
 
+/* The same step, one kernel at a time (orders 4..7): chorus_step_begin fixes dt and the scheme and makes sure the face traces
+ * of the current state exist; then, for istage = 0 .. nstages-1, chorus_stage_main launches the element kernel of the stage and
+ * chorus_stage_face finishes it (the viscous face kernel with diffusion; without diffusion it only completes the bookkeeping).
+ * After the last chorus_stage_face the new state is current.  chorus_step(dt, nstages) is exactly this sequence.  Calls out of
+ * sequence return CHORUS_ESTATE.  A partition (below) exchanges its halo between these calls. */
+int chorus_step_begin(chorus_ctx* ctx, double dt, int nstages);
+int chorus_stage_main(chorus_ctx* ctx, int istage);
+int chorus_stage_face(chorus_ctx* ctx, int istage);
+
+/* ---- element partitions for multi-GPU runs ----
+ * A rank's local mesh lists the elements it OWNS first, then GHOST copies of the off-rank face neighbours of owned elements
+ * (connectivity of owned elements refers to local indices; that of ghosts is ignored).  chorus_set_owned(n_owned) makes the
+ * context advance elements [0, n_owned) only.  Two kinds of face data of ghosts come from their owners, every stage:
+ *   field 0  face traces of the state being evaluated, 9 n^2 doubles per face   -- before chorus_stage_main
+ *   field 1  own-side viscous face fluxes, 7 n^2 doubles per face (diffusion)    -- between chorus_stage_main and _face
+ * chorus_halo_setup takes the faces to send (owned element, face) and to receive (ghost element, face), HOST arrays that are
+ * copied; chorus_halo_pack gathers the send faces of a field into buf [n_send][w n^2] and chorus_halo_unpack scatters
+ * buf [n_recv][w n^2] into the ghosts (DEVICE buffers, asynchronous on the context's stream; w = 9 or 7).  How the buffers
+ * travel (NCCL all-to-all over NVLink, peer copies) is the caller's business: paper_2502_17805_b200/partition.py.
+ * chorus_max_wavespeed and chorus_diagnostics_sums of a partition cover its owned elements; state arrays keep the local
+ * layout [9][n_elem][n^3] (ghost slots are ignored on input and meaningless on output). */
+int chorus_set_owned(chorus_ctx* ctx, int64_t n_owned);
+int chorus_halo_setup(chorus_ctx* ctx, int64_t n_send, const int32_t* send_elem, const uint8_t* send_face, int64_t n_recv,
+                      const int32_t* recv_elem, const uint8_t* recv_face);
+int chorus_halo_pack(chorus_ctx* ctx, int field, double* buf);
+int chorus_halo_unpack(chorus_ctx* ctx, int field, const double* buf);
+/* out (HOST, 3 doubles) = int dV, int 1/2 rho U.U dV, int 1/2 B.B dV over the owned elements (the undivided sums of
+ * chorus_diagnostics, to be added over the partitions). */
+int chorus_diagnostics_sums(chorus_ctx* ctx, double* out);
+
 /* *out (HOST) = max over solution points of |U| + sqrt((gamma p + |B|^2)/rho): the fast magnetosonic speed
  * maximised over direction, for the CFL condition.  Synchronises.  CHORUS_ESTATE if it is not finite. */
 int chorus_max_wavespeed(chorus_ctx* ctx, double* out);

@@ -18,7 +18,8 @@ CHORUS_OK, CHORUS_EINVAL, CHORUS_ENOMEM, CHORUS_ECUDA, CHORUS_ESTATE = 0, -1, -2
 
 # every symbol include/chorus.h declares
 SYMBOLS = ("chorus_init", "chorus_free", "chorus_set_physics", "chorus_set_state", "chorus_get_state", "chorus_residual",
-           "chorus_step", "chorus_max_wavespeed", "chorus_diagnostics", "chorus_last_error", "chorus_get_geometry", "chorus_get_gradient",
+           "chorus_step", "chorus_step_begin", "chorus_stage_main", "chorus_stage_face", "chorus_set_owned", "chorus_halo_setup",
+           "chorus_halo_pack", "chorus_halo_unpack", "chorus_diagnostics_sums", "chorus_max_wavespeed", "chorus_diagnostics", "chorus_last_error", "chorus_get_geometry", "chorus_get_gradient",
            "chorus_get_operators", "chorus_launch_count", "chorus_profile", "chorus_profile_read", "chorus_fp64_peak")
 
 
@@ -74,6 +75,14 @@ def lib():
         L.chorus_step.argtypes = [V, D, I]
         L.chorus_max_wavespeed.argtypes = [V, C.POINTER(D)]
         L.chorus_diagnostics.argtypes = [V, V]
+        L.chorus_diagnostics_sums.argtypes = [V, V]
+        L.chorus_step_begin.argtypes = [V, D, I]
+        L.chorus_stage_main.argtypes = [V, I]
+        L.chorus_stage_face.argtypes = [V, I]
+        L.chorus_set_owned.argtypes = [V, C.c_int64]
+        L.chorus_halo_setup.argtypes = [V, C.c_int64, V, V, C.c_int64, V, V]
+        L.chorus_halo_pack.argtypes = [V, I, V]
+        L.chorus_halo_unpack.argtypes = [V, I, V]
         L.chorus_last_error.argtypes = [V]
         L.chorus_last_error.restype = C.c_char_p
         L.chorus_get_geometry.argtypes = [V, V, V, V, V, I]
@@ -193,6 +202,37 @@ class Chorus:
 
     def step(self, dt, nstages=5):
         self._check(lib().chorus_step(self._ctx, float(dt), int(nstages)))
+
+    def step_begin(self, dt, nstages=5):
+        self._check(lib().chorus_step_begin(self._ctx, float(dt), int(nstages)))
+
+    def stage_main(self, istage):
+        self._check(lib().chorus_stage_main(self._ctx, int(istage)))
+
+    def stage_face(self, istage):
+        self._check(lib().chorus_stage_face(self._ctx, int(istage)))
+
+    def set_owned(self, n_owned):
+        self._check(lib().chorus_set_owned(self._ctx, int(n_owned)))
+
+    def halo_setup(self, send_elem, send_face, recv_elem, recv_face):
+        se, sf = np.ascontiguousarray(send_elem, np.int32), np.ascontiguousarray(send_face, np.uint8)
+        re_, rf = np.ascontiguousarray(recv_elem, np.int32), np.ascontiguousarray(recv_face, np.uint8)
+        assert se.size == sf.size and re_.size == rf.size
+        ps = [a.ctypes.data_as(C.c_void_p) if a.size else None for a in (se, sf, re_, rf)]
+        self._check(lib().chorus_halo_setup(self._ctx, se.size, ps[0], ps[1], re_.size, ps[2], ps[3]))
+
+    def halo_pack(self, field, buf):
+        """buf: torch CUDA float64 tensor [n_send, w n^2] (w = 9 traces, 7 viscous)."""
+        self._check(lib().chorus_halo_pack(self._ctx, int(field), C.c_void_p(buf.data_ptr())))
+
+    def halo_unpack(self, field, buf):
+        self._check(lib().chorus_halo_unpack(self._ctx, int(field), C.c_void_p(buf.data_ptr())))
+
+    def diagnostics_sums(self):
+        out = np.empty(3)
+        self._check(lib().chorus_diagnostics_sums(self._ctx, out.ctypes.data_as(C.c_void_p)))
+        return out
 
     def max_wavespeed(self):
         v = C.c_double()

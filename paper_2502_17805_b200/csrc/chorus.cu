@@ -23,7 +23,8 @@ using namespace chorus;
 
 struct chorus_ctx {
   int n = 0, n2 = 0, n3 = 0, nf = 0;
-  int64_t E = 0;
+  int64_t E = 0;          // elements of the local mesh: the owned ones first, then the ghosts of a partition
+  int64_t E_own = 0;      // elements this context advances (= E unless chorus_set_owned made it a partition)
   cudaStream_t stream = nullptr;
   chorus_physics phys{};
   PhysD ph{};
@@ -49,6 +50,16 @@ struct chorus_ctx {
   unsigned long long* d_ws = nullptr;
   double *d_wq = nullptr, *d_diag = nullptr;   // quadrature weights [n]; diagnostics partial sums [kDiagBlocks + 1][3]
   unsigned* d_arrivals = nullptr;   // per-SM CTA arrival counters of the main kernel
+  // partition halo (chorus_halo_setup): faces whose traces / viscous fluxes go to, and come from, other partitions
+  int64_t n_send = 0, n_recv = 0;
+  int32_t *d_send_elem = nullptr, *d_recv_elem = nullptr;
+  uint8_t *d_send_face = nullptr, *d_recv_face = nullptr;
+  // split step (chorus_step_begin / chorus_stage_main / chorus_stage_face)
+  double split_dt = 0.0;
+  int split_nstages = 0, split_next = -1;   // next stage to run (-1: no split step in progress)
+  bool split_face_pending = false;
+  int split_b[5] = {0, 0, 0, 0, 0};
+  StageIO pend{};
   double* d_scratch = nullptr;      // per-CTA global scratch of the scalar kernels' SPILL variants (orders 8, 9 with diffusion)
   size_t scratch_doubles = 0;
   int64_t launches = 0;
@@ -163,10 +174,10 @@ struct Hot {
       CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, threads, smem));
       if (occ < 1) occ = 1;
       const int64_t cap = (int64_t)c->num_sms * occ;
-      const int grid = (int)(c->E < cap ? c->E : cap);
+      const int grid = (int)(c->E_own < cap ? c->E_own : cap);
       {
         ProfScope ps(c, 2);
-        k<<<grid, threads, smem, c->stream>>>(c->E, c->ph, io, geo(c));
+        k<<<grid, threads, smem, c->stream>>>(c->E_own, c->ph, io, geo(c));
       }
       ++c->launches;
       CU(c, cudaGetLastError());
@@ -183,10 +194,10 @@ struct Hot {
     CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, smem));
     if (occ < 1) occ = 1;
     const int64_t cap = (int64_t)c->num_sms * occ;
-    const int grid = (int)(c->E < cap ? c->E : cap);
+    const int grid = (int)(c->E_own < cap ? c->E_own : cap);
     {
       ProfScope ps(c, 1);
-      k<<<grid, 256, smem, c->stream>>>(c->E, io, geo(c));
+      k<<<grid, 256, smem, c->stream>>>(c->E_own, io, geo(c));
     }
     ++c->launches;
     CU(c, cudaGetLastError());
@@ -196,22 +207,23 @@ struct Hot {
     return Geo{c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl, c->d_nfc, c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient};
   }
   // one residual evaluation through the pipeline.  io carries Qe and the outputs; the traces of Qe must be in d_Qf[qf_cur].
-  static int stage_pipeline(chorus_ctx* c, StageIO io) {
+  static int stage_pipeline_main(chorus_ctx* c, StageIO& io) {
     io.Qf = c->d_Qf[c->qf_cur];
     io.QfOut = c->d_Qf[c->qf_cur ^ 1];
     io.Vf = c->d_Vf;
     const int gv = gradv_of(c->phys);
-    int rc;
-    if (gv == 2) {
-      if ((rc = main_launch<true, 2>(c, io))) return rc;
-      rc = face_launch(c, io);
-    } else if (gv == 1) {
-      rc = main_launch<false, 1>(c, io);
-    } else {
-      rc = main_launch<false, 0>(c, io);
-    }
+    if (gv == 2) return main_launch<true, 2>(c, io);
+    if (gv == 1) return main_launch<false, 1>(c, io);
+    return main_launch<false, 0>(c, io);
+  }
+  static int stage_pipeline_face(chorus_ctx* c, const StageIO& io) {
+    int rc = gradv_of(c->phys) == 2 ? face_launch(c, io) : CHORUS_OK;
     if (!rc && io.Qout != nullptr) c->qf_cur ^= 1;   // the traces of the new state were emitted into the other buffer
     return rc;
+  }
+  static int stage_pipeline(chorus_ctx* c, StageIO io) {
+    int rc = stage_pipeline_main(c, io);
+    return rc ? rc : stage_pipeline_face(c, io);
   }
   static int trace(chorus_ctx* c, const double* Qin, double* Qf) {
     constexpr size_t smem = sizeof(double) * 9 * I::n3;
@@ -221,10 +233,10 @@ struct Hot {
     CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, smem));
     if (occ < 1) occ = 1;
     const int64_t cap = (int64_t)c->num_sms * occ;
-    const int grid = (int)(c->E < cap ? c->E : cap);
+    const int grid = (int)(c->E_own < cap ? c->E_own : cap);
     {
       ProfScope ps(c, 0);
-      k<<<grid, 256, smem, c->stream>>>(c->E, Qin, Qf);
+      k<<<grid, 256, smem, c->stream>>>(c->E_own, Qin, Qf);
     }
     ++c->launches;
     CU(c, cudaGetLastError());
@@ -275,8 +287,20 @@ struct Hot {
   }
   // one residual evaluation of the state in Qin, fused with the output / RK combination described by `out`.
   // scratch: a state-sized buffer distinct from Qin, the outputs and the stage registers (residual mode with diffusion).
-  static int stage(chorus_ctx* c, const double* Qin, const StageOut& out, double* scratch) {
-    if (!(c->use_mma && N >= 4 && N <= 7)) return stage_legacy(c, Qin, out);
+  // split: only the element kernel is launched and the stage is left pending in c->pend (chorus_stage_main); face_pending()
+  // finishes it (chorus_stage_face).  A partition exchanges halo data between the two.
+  static int face_pending(chorus_ctx* c) { return stage_pipeline_face(c, c->pend); }
+  static int ensure_traces(chorus_ctx* c, const double* Qin) {
+    if (!(c->use_mma && N >= 4 && N <= 7)) return fail(c, CHORUS_EINVAL, "the split step serves the DMMA pipeline (orders 4..7)");
+    if (!c->traces_valid) {
+      int rc = trace(c, Qin, c->d_Qf[c->qf_cur]);
+      if (rc) return rc;
+      c->traces_valid = true;
+    }
+    return CHORUS_OK;
+  }
+  static int stage(chorus_ctx* c, const double* Qin, const StageOut& out, double* scratch, bool split = false) {
+    if (!(c->use_mma && N >= 4 && N <= 7)) return split ? fail(c, CHORUS_EINVAL, "the split step serves orders 4..7") : stage_legacy(c, Qin, out);
     if (!c->traces_valid) {
       int rc = trace(c, Qin, c->d_Qf[c->qf_cur]);
       if (rc) return rc;
@@ -300,6 +324,11 @@ struct Hot {
         else if (k == 1) { io.A1 = A[i]; io.c1 = cc[i]; ++k; }
         else return fail(c, CHORUS_EINVAL, "more than two foreign stage registers");
       }
+    }
+    if (split) {
+      int rc = stage_pipeline_main(c, io);
+      c->pend = io;
+      return rc;
     }
     return stage_pipeline(c, io);
   }
@@ -380,6 +409,7 @@ int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chor
   if (!c) return CHORUS_ENOMEM;
   c->n = order; c->n2 = order * order; c->n3 = c->n2 * order; c->nf = c->n2 * (order + 1);
   c->E = mesh->n_elem;
+  c->E_own = mesh->n_elem;
   c->ng = mesh->n_geom;
   c->stream = (cudaStream_t)cuda_stream;
   c->phys = *phys;
@@ -444,7 +474,8 @@ void chorus_free(chorus_ctx* c) {
   cudaFree(c->d_Gm); cudaFree(c->d_Dff); cudaFree(c->d_Efs); cudaFree(c->d_Dfs);
   cudaFree(c->d_Sfl); cudaFree(c->d_detJ); cudaFree(c->d_jinv); cudaFree(c->d_xsol); cudaFree(c->d_krfl); cudaFree(c->d_nfc);
   for (int k = 0; k < 5; ++k) cudaFree(c->d_U[k]);
-  cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_ws); cudaFree(c->d_wq); cudaFree(c->d_diag); cudaFree(c->d_arrivals); cudaFree(c->d_scratch);
+  cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_send_elem); cudaFree(c->d_send_face); cudaFree(c->d_recv_elem); cudaFree(c->d_recv_face);
+  cudaFree(c->d_ws); cudaFree(c->d_wq); cudaFree(c->d_diag); cudaFree(c->d_arrivals); cudaFree(c->d_scratch);
   for (auto& v : c->prof_ev)
     for (auto& ev : v) {
       cudaEventDestroy(ev.first);
@@ -504,6 +535,8 @@ int chorus_get_state(chorus_ctx* c, double* q, int on_device) {
 int chorus_residual(chorus_ctx* c, double* r, int on_device) {
   if (!c || !r) return CHORUS_EINVAL;
   if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
+  if (c->E_own != c->E) return fail(c, CHORUS_EINVAL, "chorus_residual serves whole meshes; a partition advances through the split step");
+  if (c->split_next >= 0) return fail(c, CHORUS_ESTATE, "a split step is in progress");
   const size_t count = (size_t)c->E * 9 * c->n3;
   StageOut o{};
   o.Rout = on_device ? r : c->d_U[(c->cur + 1) % 5];
@@ -518,36 +551,30 @@ int chorus_residual(chorus_ctx* c, double* r, int on_device) {
   return CHORUS_OK;
 }
 
-int chorus_step(chorus_ctx* c, double dt, int nstages) {
-  if (!c || (nstages != 1 && nstages != 3 && nstages != 5) || !(dt == dt)) return c ? fail(c, CHORUS_EINVAL, "bad dt or nstages") : CHORUS_EINVAL;
-  if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
-  int b[5];
-  for (int k = 0; k < 5; ++k) b[k] = (c->cur + k) % 5;
-  double** U = c->d_U;
-  auto run = [&](int in, int outb, const double* A0, double c0, const double* A1, double c1, const double* A2, double c2, double bdt) {
-    StageOut o{};
-    o.Qout = U[outb];
-    o.A0 = A0; o.A1 = A1; o.A2 = A2;
-    o.c0 = c0; o.c1 = c1; o.c2 = c2; o.bdt = bdt;
-    const double* Qin = U[in];
-    return DISPATCH_N(c, H::stage(c, Qin, o, nullptr));
+namespace {
+// Stage i (0-based) of an nstages-stage step of size dt on the register ring b[0..4] (b[0] holds the current state):
+// which register is evaluated, which receives  sum_k c_k U[A_k] + bdt * R(U[in]),  and which register is current afterwards.
+struct StageArgs {
+  int in, outb, cur_after;
+  const double *A0, *A1, *A2;
+  double c0, c1, c2, bdt;
+};
+bool stage_args(const chorus_ctx* c, int nstages, int i, double dt, const int* b, StageArgs& a) {
+  double* const* U = c->d_U;
+  a = StageArgs{0, 0, 0, nullptr, nullptr, nullptr, 0.0, 0.0, 0.0, 0.0};
+  auto set = [&](int in, int outb, const double* A0, double c0, const double* A1, double c1, const double* A2, double c2, double bdt) {
+    a.in = b[in]; a.outb = b[outb]; a.A0 = A0; a.c0 = c0; a.A1 = A1; a.c1 = c1; a.A2 = A2; a.c2 = c2; a.bdt = bdt;
+    a.cur_after = b[outb];
   };
-  int rc = 0;
-  // a stage that fails leaves the trace buffers describing an intermediate state: they must not be reused
-  struct TraceGuard {
-    chorus_ctx* c;
-    bool ok = false;
-    ~TraceGuard() { if (!ok) c->traces_valid = false; }
-  } guard{c};
   if (nstages == 1) {
-    if ((rc = run(b[0], b[1], U[b[0]], 1.0, nullptr, 0, nullptr, 0, dt))) return rc;
-    c->cur = b[1];
+    if (i != 0) return false;
+    set(0, 1, U[b[0]], 1.0, nullptr, 0, nullptr, 0, dt);
   } else if (nstages == 3) {   // Shu-Osher SSPRK(3,3)
-    if ((rc = run(b[0], b[1], U[b[0]], 1.0, nullptr, 0, nullptr, 0, dt))) return rc;
-    if ((rc = run(b[1], b[2], U[b[0]], 0.75, U[b[1]], 0.25, nullptr, 0, 0.25 * dt))) return rc;
-    if ((rc = run(b[2], b[3], U[b[0]], 1.0 / 3.0, U[b[2]], 2.0 / 3.0, nullptr, 0, (2.0 / 3.0) * dt))) return rc;
-    c->cur = b[3];
-  } else {
+    if (i == 0) set(0, 1, U[b[0]], 1.0, nullptr, 0, nullptr, 0, dt);
+    else if (i == 1) set(1, 2, U[b[0]], 0.75, U[b[1]], 0.25, nullptr, 0, 0.25 * dt);
+    else if (i == 2) set(2, 3, U[b[0]], 1.0 / 3.0, U[b[2]], 2.0 / 3.0, nullptr, 0, (2.0 / 3.0) * dt);
+    else return false;
+  } else if (nstages == 5) {
     // SSPRK(5,3) of Ruuth in Shu-Osher form; F(u0) and F(u1) of stages 4 and 5 are eliminated through
     // dt F(u0) = (u1 - u0)/beta1 and dt F(u1) = (u2 - u1)/beta1, so only state registers are kept.
     const double be1 = 0.37726891511710;
@@ -558,24 +585,158 @@ int chorus_step(chorus_ctx* c, double dt, int nstages) {
     const double c40 = a40 - b40 / be1, c41 = a41 + b40 / be1;
     const double c50 = a50 - b50 / be1, c51 = a51 + b50 / be1 - b51 / be1, c52 = a52 + b51 / be1;
     (void)c50;   // = -4e-16: u0's weight in stage 5 cancels to round-off and is dropped
-    if ((rc = run(b[0], b[1], U[b[0]], 1.0, nullptr, 0, nullptr, 0, be1 * dt))) return rc;
-    if ((rc = run(b[1], b[2], U[b[1]], 1.0, nullptr, 0, nullptr, 0, be1 * dt))) return rc;
-    if ((rc = run(b[2], b[3], U[b[0]], a30, U[b[2]], a32, nullptr, 0, b32 * dt))) return rc;
-    if ((rc = run(b[3], b[4], U[b[0]], c40, U[b[1]], c41, U[b[3]], a43, b43 * dt))) return rc;
-    if ((rc = run(b[4], b[0], U[b[1]], c51, U[b[2]], c52, U[b[4]], a54, b54 * dt))) return rc;
-    c->cur = b[0];
+    if (i == 0) set(0, 1, U[b[0]], 1.0, nullptr, 0, nullptr, 0, be1 * dt);
+    else if (i == 1) set(1, 2, U[b[1]], 1.0, nullptr, 0, nullptr, 0, be1 * dt);
+    else if (i == 2) set(2, 3, U[b[0]], a30, U[b[2]], a32, nullptr, 0, b32 * dt);
+    else if (i == 3) set(3, 4, U[b[0]], c40, U[b[1]], c41, U[b[3]], a43, b43 * dt);
+    else if (i == 4) set(4, 0, U[b[1]], c51, U[b[2]], c52, U[b[4]], a54, b54 * dt);
+    else return false;
+  } else {
+    return false;
   }
+  return true;
+}
+int run_stage(chorus_ctx* c, const StageArgs& a, bool split) {
+  StageOut o{};
+  o.Qout = c->d_U[a.outb];
+  o.A0 = a.A0; o.A1 = a.A1; o.A2 = a.A2;
+  o.c0 = a.c0; o.c1 = a.c1; o.c2 = a.c2; o.bdt = a.bdt;
+  const double* Qin = c->d_U[a.in];
+  return DISPATCH_N(c, H::stage(c, Qin, o, nullptr, split));
+}
+}  // namespace
+
+int chorus_step(chorus_ctx* c, double dt, int nstages) {
+  if (!c || (nstages != 1 && nstages != 3 && nstages != 5) || !(dt == dt)) return c ? fail(c, CHORUS_EINVAL, "bad dt or nstages") : CHORUS_EINVAL;
+  if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
+  if (c->E_own != c->E) return fail(c, CHORUS_EINVAL, "a partition steps through chorus_step_begin / chorus_stage_main / chorus_stage_face");
+  if (c->split_next >= 0) return fail(c, CHORUS_ESTATE, "a split step is in progress");
+  int b[5];
+  for (int k = 0; k < 5; ++k) b[k] = (c->cur + k) % 5;
+  // a stage that fails leaves the trace buffers describing an intermediate state: they must not be reused
+  struct TraceGuard {
+    chorus_ctx* c;
+    bool ok = false;
+    ~TraceGuard() { if (!ok) c->traces_valid = false; }
+  } guard{c};
+  StageArgs a;
+  for (int i = 0; i < nstages; ++i) {
+    stage_args(c, nstages, i, dt, b, a);
+    int rc = run_stage(c, a, false);
+    if (rc) return rc;
+  }
+  c->cur = a.cur_after;
   guard.ok = true;
   return CHORUS_OK;
 }
+
+// ---- the same step, one kernel at a time (what a partition's driver interleaves with its halo exchanges)
+int chorus_step_begin(chorus_ctx* c, double dt, int nstages) {
+  if (!c || (nstages != 1 && nstages != 3 && nstages != 5) || !(dt == dt)) return c ? fail(c, CHORUS_EINVAL, "bad dt or nstages") : CHORUS_EINVAL;
+  if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
+  if (c->split_next >= 0) return fail(c, CHORUS_ESTATE, "a split step is already in progress");
+  const double* Qin = c->d_U[c->cur];
+  int rc = DISPATCH_N(c, H::ensure_traces(c, Qin));
+  if (rc) return rc;
+  for (int k = 0; k < 5; ++k) c->split_b[k] = (c->cur + k) % 5;
+  c->split_dt = dt;
+  c->split_nstages = nstages;
+  c->split_next = 0;
+  c->split_face_pending = false;
+  return CHORUS_OK;
+}
+
+int chorus_stage_main(chorus_ctx* c, int istage) {
+  if (!c) return CHORUS_EINVAL;
+  if (c->split_next < 0 || istage != c->split_next || c->split_face_pending) return fail(c, CHORUS_ESTATE, "chorus_stage_main out of sequence");
+  StageArgs a;
+  if (!stage_args(c, c->split_nstages, istage, c->split_dt, c->split_b, a)) return fail(c, CHORUS_EINVAL, "bad stage index");
+  int rc = run_stage(c, a, true);
+  if (rc) {
+    c->traces_valid = false;
+    c->split_next = -1;
+    return rc;
+  }
+  c->split_face_pending = true;
+  return CHORUS_OK;
+}
+
+int chorus_stage_face(chorus_ctx* c, int istage) {
+  if (!c) return CHORUS_EINVAL;
+  if (c->split_next < 0 || istage != c->split_next || !c->split_face_pending) return fail(c, CHORUS_ESTATE, "chorus_stage_face out of sequence");
+  int rc = DISPATCH_N(c, H::face_pending(c));
+  c->split_face_pending = false;
+  if (rc) {
+    c->traces_valid = false;
+    c->split_next = -1;
+    return rc;
+  }
+  if (istage + 1 == c->split_nstages) {
+    StageArgs a;
+    stage_args(c, c->split_nstages, istage, c->split_dt, c->split_b, a);
+    c->cur = a.cur_after;
+    c->split_next = -1;
+  } else {
+    c->split_next = istage + 1;
+  }
+  return CHORUS_OK;
+}
+
+// ---- partitions: owned elements first, ghosts after; halo faces packed into / unpacked from contiguous device buffers
+int chorus_set_owned(chorus_ctx* c, int64_t n_owned) {
+  if (!c || n_owned < 1 || n_owned > c->E) return c ? fail(c, CHORUS_EINVAL, "n_owned must be in 1..n_elem") : CHORUS_EINVAL;
+  c->E_own = n_owned;
+  c->traces_valid = false;
+  return CHORUS_OK;
+}
+
+int chorus_halo_setup(chorus_ctx* c, int64_t n_send, const int32_t* send_elem, const uint8_t* send_face, int64_t n_recv,
+                      const int32_t* recv_elem, const uint8_t* recv_face) {
+  if (!c || n_send < 0 || n_recv < 0 || (n_send && (!send_elem || !send_face)) || (n_recv && (!recv_elem || !recv_face))) return CHORUS_EINVAL;
+  for (int64_t k = 0; k < n_send; ++k)
+    if (send_elem[k] < 0 || send_elem[k] >= c->E_own || send_face[k] > 5) return fail(c, CHORUS_EINVAL, "halo send list: owned element and face 0..5");
+  for (int64_t k = 0; k < n_recv; ++k)
+    if (recv_elem[k] < c->E_own || recv_elem[k] >= c->E || recv_face[k] > 5) return fail(c, CHORUS_EINVAL, "halo receive list: ghost element and face 0..5");
+  cudaFree(c->d_send_elem); cudaFree(c->d_send_face); cudaFree(c->d_recv_elem); cudaFree(c->d_recv_face);
+  c->d_send_elem = c->d_recv_elem = nullptr;
+  c->d_send_face = c->d_recv_face = nullptr;
+  c->n_send = c->n_recv = 0;
+  int rc = 0;
+  if (n_send && ((rc = upload(c, &c->d_send_elem, send_elem, (size_t)n_send)) || (rc = upload(c, &c->d_send_face, send_face, (size_t)n_send)))) return rc;
+  if (n_recv && ((rc = upload(c, &c->d_recv_elem, recv_elem, (size_t)n_recv)) || (rc = upload(c, &c->d_recv_face, recv_face, (size_t)n_recv)))) return rc;
+  CU(c, cudaStreamSynchronize(c->stream));   // the host lists may be released by the caller
+  c->n_send = n_send;
+  c->n_recv = n_recv;
+  return CHORUS_OK;
+}
+
+namespace {
+// field 0: face traces of the current state (9 n^2 doubles per face); field 1: own-side viscous face fluxes (7 n^2)
+int halo_copy(chorus_ctx* c, int field, double* buf, bool pack) {
+  if (!c || (field != 0 && field != 1) || !buf) return c ? fail(c, CHORUS_EINVAL, "halo field 0 (traces) or 1 (viscous face fluxes)") : CHORUS_EINVAL;
+  const int64_t cnt = pack ? c->n_send : c->n_recv;
+  if (cnt == 0) return CHORUS_OK;
+  const int w = (field == 0 ? 9 : 7) * c->n2;
+  double* base = field == 0 ? c->d_Qf[c->qf_cur] : c->d_Vf;
+  const int32_t* el = pack ? c->d_send_elem : c->d_recv_elem;
+  const uint8_t* fc = pack ? c->d_send_face : c->d_recv_face;
+  halo_copy_kernel<<<grid_1d(c, cnt * w, 256), 256, 0, c->stream>>>(cnt, w, el, fc, base, buf, pack ? 1 : 0);
+  ++c->launches;
+  CU(c, cudaGetLastError());
+  return CHORUS_OK;
+}
+}  // namespace
+
+int chorus_halo_pack(chorus_ctx* c, int field, double* buf) { return halo_copy(c, field, buf, true); }
+int chorus_halo_unpack(chorus_ctx* c, int field, const double* buf) { return halo_copy(c, field, const_cast<double*>(buf), false); }
 
 int chorus_max_wavespeed(chorus_ctx* c, double* out) {
   if (!c || !out) return CHORUS_EINVAL;
   if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
   CU(c, cudaMemsetAsync(c->d_ws, 0, sizeof(unsigned long long), c->stream));
-  const int64_t total = c->E * c->n3;
+  const int64_t total = c->E_own * c->n3;
   int grid = grid_1d(c, total, 256);
-  wavespeed_kernel<<<grid, 256, 0, c->stream>>>(c->E, c->n3, c->ph, c->d_U[c->cur], c->d_ws);
+  wavespeed_kernel<<<grid, 256, 0, c->stream>>>(c->E_own, c->n3, c->ph, c->d_U[c->cur], c->d_ws);
   ++c->launches;
   CU(c, cudaGetLastError());
   unsigned long long bits = 0;
@@ -588,21 +749,25 @@ int chorus_max_wavespeed(chorus_ctx* c, double* out) {
   return CHORUS_OK;
 }
 
-int chorus_diagnostics(chorus_ctx* c, double* out) {
+namespace {
+int diagnostics_impl(chorus_ctx* c, double* out, bool sums) {
   if (!c || !out) return CHORUS_EINVAL;
   if (!c->have_state) return fail(c, CHORUS_ESTATE, "no state set");
-  const int64_t total = c->E * c->n3;
+  const int64_t total = c->E_own * c->n3;
   const int grid = (int)std::min<int64_t>(kDiagBlocks, (total + 255) / 256);
-  diagnostics_kernel<<<grid, 256, 0, c->stream>>>(c->E, c->n, c->d_wq, c->d_detJ, c->d_U[c->cur], c->d_diag);
+  diagnostics_kernel<<<grid, 256, 0, c->stream>>>(c->E_own, c->n, c->d_wq, c->d_detJ, c->d_U[c->cur], c->d_diag);
   ++c->launches;
   CU(c, cudaGetLastError());
-  diagnostics_final_kernel<<<1, 256, 0, c->stream>>>(grid, c->d_diag, c->d_diag + (size_t)kDiagBlocks * 3);
+  diagnostics_final_kernel<<<1, 256, 0, c->stream>>>(grid, c->d_diag, c->d_diag + (size_t)kDiagBlocks * 3, sums ? 1 : 0);
   ++c->launches;
   CU(c, cudaGetLastError());
   CU(c, cudaMemcpyAsync(out, c->d_diag + (size_t)kDiagBlocks * 3, sizeof(double) * 3, cudaMemcpyDeviceToHost, c->stream));
   CU(c, cudaStreamSynchronize(c->stream));
   return CHORUS_OK;
 }
+}  // namespace
+int chorus_diagnostics(chorus_ctx* c, double* out) { return diagnostics_impl(c, out, false); }
+int chorus_diagnostics_sums(chorus_ctx* c, double* out) { return diagnostics_impl(c, out, true); }
 
 int chorus_get_geometry(chorus_ctx* c, double* detJ, double* S, double* xsol, double* jinv, int on_device) {
   if (!c) return CHORUS_EINVAL;

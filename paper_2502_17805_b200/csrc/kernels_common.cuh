@@ -206,12 +206,30 @@ __global__ void __launch_bounds__(256) diagnostics_kernel(int64_t E, int n, cons
   block_sum3(V, KE, EB, sh);
   if (threadIdx.x == 0) { partial[blockIdx.x * 3 + 0] = V; partial[blockIdx.x * 3 + 1] = KE; partial[blockIdx.x * 3 + 2] = EB; }
 }
-__global__ void __launch_bounds__(256) diagnostics_final_kernel(int nparts, const double* __restrict__ partial, double* __restrict__ out /*[3]*/) {
+// sums != 0: the raw integrals (a partition's share; the caller adds the partitions' and divides)
+__global__ void __launch_bounds__(256) diagnostics_final_kernel(int nparts, const double* __restrict__ partial, double* __restrict__ out /*[3]*/,
+                                                               int sums) {
   __shared__ double sh[8][3];
   double V = 0.0, KE = 0.0, EB = 0.0;
   for (int t = threadIdx.x; t < nparts; t += blockDim.x) { V += partial[t * 3]; KE += partial[t * 3 + 1]; EB += partial[t * 3 + 2]; }
   block_sum3(V, KE, EB, sh);
-  if (threadIdx.x == 0) { out[0] = V; out[1] = KE / V; out[2] = EB / V; }
+  if (threadIdx.x == 0) { out[0] = V; out[1] = sums ? KE : KE / V; out[2] = sums ? EB : EB / V; }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Halo of a partition: item k is face fc[k] of element el[k]; its block of w doubles (9 n^2 face traces or
+// 7 n^2 viscous face fluxes) at base[(el*6 + fc) * w] is copied to (pack) or from (unpack) buf[k * w].
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) halo_copy_kernel(int64_t cnt, int w, const int32_t* __restrict__ el, const uint8_t* __restrict__ fc,
+                                                       double* __restrict__ base, double* __restrict__ buf, int pack) {
+  const int64_t total = cnt * w;
+  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t k = t / w;
+    const int j = (int)(t % w);
+    double* p = base + ((int64_t)el[k] * 6 + fc[k]) * w + j;
+    if (pack) buf[t] = *p;
+    else *p = buf[t];
+  }
 }
 
 }  // namespace chorus

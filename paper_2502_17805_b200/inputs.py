@@ -548,3 +548,70 @@ def extract_patch(mesh: dict, center: int, rings: int = 2):
                nbr_face=np.ascontiguousarray(mesh["nbr_face"][elems]), nbr_orient=np.ascontiguousarray(mesh["nbr_orient"][elems]),
                kind="patch")
     return out, elems
+
+
+# --------------------------------------------------------------------------------------
+# element partitions for multi-GPU runs: contiguous blocks of the element order; every rank's local
+# mesh = its owned elements followed by ghost copies of their off-rank face neighbours, plus the lists of faces whose
+# data cross between ranks.  Pure indexing: no arithmetic of the method.
+# --------------------------------------------------------------------------------------
+def partition_mesh(mesh: dict, n_parts: int, rank: int | None = None):
+    """Split `mesh` into n_parts partitions (rank p owns the global elements [E p / P, E (p+1) / P)).
+
+    Returns a list of partition dicts (or the one of `rank`), each with
+      mesh        local mesh dict: owned elements [0, n_owned) then ghosts; nbr_elem of owned elements holds local indices
+                  (ghost faces of ghosts are closed with -2 and never used)
+      n_owned     number of owned elements
+      elems       int64[n_local]: global element of every local element (owned then ghosts, ghosts in increasing order)
+      send_elem, send_face, send_counts   faces of owned elements whose data other ranks need, grouped by destination rank
+                  in increasing rank order (send_counts[q] items go to rank q), each group sorted by (global element, face)
+      recv_elem, recv_face, recv_counts   the matching faces of ghost elements, grouped by source rank, same order
+    The face (g, f) of an element g owned by q is needed by p when the element across f is owned by p != q."""
+    E = int(mesh["n_elem"])
+    P = int(n_parts)
+    if P < 1 or P > E:
+        raise ValueError("need 1 <= n_parts <= n_elem")
+    bounds = [E * p // P for p in range(P + 1)]
+    owner = np.empty(E, np.int64)
+    for p in range(P):
+        owner[bounds[p]:bounds[p + 1]] = p
+    nbr, nface = mesh["nbr_elem"], mesh["nbr_face"]
+    parts = []
+    for p in (range(P) if rank is None else [int(rank)]):
+        lo, hi = bounds[p], bounds[p + 1]
+        own = np.arange(lo, hi)
+        ne = nbr[lo:hi]                                             # [n_owned, 6]
+        off = (ne >= 0) & ((ne < lo) | (ne >= hi))
+        ghosts = np.unique(ne[off])
+        elems = np.concatenate([own, ghosts]).astype(np.int64)
+        local = {int(g): i for i, g in enumerate(elems)}
+        pe = np.full((elems.size, 6), -2, np.int32)
+        for i in range(hi - lo):
+            for f in range(6):
+                v = int(ne[i, f])
+                pe[i, f] = v if v < 0 else local[v]
+        pm = dict(n_elem=int(elems.size), n_geom=mesh["n_geom"], geom_nodes=mesh["geom_nodes"].copy(),
+                  xyz=np.ascontiguousarray(mesh["xyz"][elems]), nbr_elem=pe,
+                  nbr_face=np.ascontiguousarray(mesh["nbr_face"][elems]), nbr_orient=np.ascontiguousarray(mesh["nbr_orient"][elems]),
+                  kind="partition")
+        # faces crossing the partition boundary, seen from the owned side: (e, f) with the neighbour on another rank
+        ei, fi = np.nonzero(off)
+        nb_glob = ne[ei, fi]
+        nb_rank = owner[nb_glob]
+        # what WE send to rank q: our face (e, f); sorted by (destination, global e, f)
+        order = np.lexsort((fi, ei + lo, nb_rank))
+        send_elem, send_face = ei[order].astype(np.int32), fi[order].astype(np.uint8)
+        send_counts = np.bincount(nb_rank, minlength=P).astype(np.int64)
+        # what we RECEIVE from rank q: the neighbour's face (g, f'), f' = nbr_face[e, f]; sorted by (source, global g, f')
+        nb_face = nface[ei + lo, fi]
+        order = np.lexsort((nb_face, nb_glob, nb_rank))
+        recv_elem = np.array([local[int(g)] for g in nb_glob[order]], np.int32)
+        recv_face = nb_face[order].astype(np.uint8)
+        # a ghost face can be reached from one owned face only (conforming mesh), but be safe against duplicates
+        key = recv_elem.astype(np.int64) * 6 + recv_face
+        if np.unique(key).size != key.size:
+            raise ValueError("a ghost face is referenced twice: the mesh is not conforming")
+        parts.append(dict(mesh=pm, n_owned=int(hi - lo), elems=elems, rank=p, n_parts=P,
+                          send_elem=send_elem, send_face=send_face, send_counts=send_counts,
+                          recv_elem=recv_elem, recv_face=recv_face, recv_counts=send_counts.copy()))
+    return parts if rank is None else parts[0]

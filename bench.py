@@ -111,7 +111,8 @@ def workload_config(w, args, world, pts=None):
     pts = w.n_elem * w.order ** 3 if pts is None else pts
     return dict(workload=args.workload, mesh=f"6x{w.n_z}x{w.n_z}x{w.n_r} cubed-sphere shell", n_elem=w.n_elem, order=w.order,
                 solution_points=pts, N_rho=w.N_rho, diffusion=w.diffusion, rk="SSPRK(5,3)",
-                parallelism="replicas" if world > 1 else "single GPU", l2="inputs larger than L2 (state %.0f MB)" % (pts * 72 / 1e6))
+                parallelism=("single GPU" if world == 1 else f"{world} element partitions, halo all-to-all" if getattr(args, "parallel", "halo") == "halo"
+                             else f"{world} replicas"), l2="inputs larger than L2 (state %.0f MB)" % (pts * 72 / 1e6))
 
 
 class ClockSampler:
@@ -216,6 +217,9 @@ def main():
     ap.add_argument("--workload", default="config3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--parallel", default="halo", choices=["halo", "replicas"],
+                    help="N > 1: 'halo' = ONE workload split into N element partitions with halo exchange (strong scaling); "
+                         "'replicas' = every rank advances its own copy (weak scaling, no data-path collective)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
@@ -240,16 +244,25 @@ def main():
     w = I.workload(args.workload)
     n = w.order
     mesh = w.mesh()
-    g = P.Chorus(mesh, n, I.Physics())
-    Q = w.state(g.xsol())
+    halo = world > 1 and args.parallel == "halo"
+    if halo:
+        # one workload, `world` element partitions: this rank owns a contiguous block of elements plus ghost copies of its
+        # off-rank face neighbours; face traces and viscous face fluxes of the partition boundary travel by NCCL all-to-all
+        from paper_2502_17805_b200.partition import DistributedChorus
+        job = DistributedChorus(mesh, n, I.Physics(), dist)
+        g = job.g
+        pts = mesh["n_elem"] * n ** 3                 # the whole job's solution points
+    else:
+        g = job = P.Chorus(mesh, n, I.Physics())
+        pts = g.E * n ** 3
+    Q = w.state(g.xsol())                             # the local elements' state (ghost slots are ignored by a partition)
     del mesh
-    pts = g.E * n ** 3
     host = torch.from_numpy(Q).pin_memory()
     del Q
     g.set_state(host.numpy())
-    c_h = g.max_wavespeed()
+    c_h = job.max_wavespeed()
     phys = w.physics(c_h)
-    g.set_physics(phys)
+    job.set_physics(phys)
     _, xf, _, _ = P.get_operators(n)
     dt = w.dt(c_h, xf[1] - xf[0])
     diff = w.diffusion > 0
@@ -261,25 +274,25 @@ def main():
 
     # ---- device-resident throughput
     for _ in range(warmup):
-        g.step(dt, NSTAGES)
+        job.step(dt, NSTAGES)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = g.launch_count()
     barrier()
     with ClockSampler(local) as clocks:     # the headline loop: no per-launch events
         ev0.record()
         for _ in range(args.steps):
-            g.step(dt, NSTAGES)
+            job.step(dt, NSTAGES)
         ev1.record()
         barrier()
     ms = ev0.elapsed_time(ev1)
     launches = g.launch_count() - l0
-    ws_after = g.max_wavespeed()          # also proves the state is still finite
+    ws_after = job.max_wavespeed()        # also proves the state is still finite
     # ---- per-kernel device times: a separate pass with every launch bracketed by CUDA events on the library's stream
     g.profile(True)
     g.profile_read()
     prof_steps = max(1, min(args.steps, 4))
     for _ in range(prof_steps):
-        g.step(dt, NSTAGES)
+        job.step(dt, NSTAGES)
     prof = g.profile_read()
     g.profile(False)
     prof_ms = sum(v[0] for v in prof.values())
@@ -290,22 +303,22 @@ def main():
         e2e_steps = max(1, min(args.steps, 5))
         hnp = host.numpy()
         out = torch.empty_like(host).pin_memory().numpy()
-        g.set_state(hnp); g.step(dt, NSTAGES); g.get_state(out); g.max_wavespeed()
+        g.set_state(hnp); job.step(dt, NSTAGES); g.get_state(out); job.max_wavespeed()
         barrier()
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
             g.set_state(hnp)
-            g.step(dt, NSTAGES)
+            job.step(dt, NSTAGES)
             g.get_state(out)
-            g.max_wavespeed()
+            job.max_wavespeed()
         barrier()
         e2e_ms = 1e3 * (time.perf_counter() - t0)
         assert np.isfinite(out[:, ::max(1, out.shape[1] // 64)]).all()
         t0 = time.perf_counter()
         for _ in range(e2e_steps):          # the same without the state coming back (round 1's figure), for comparison
             g.set_state(hnp)
-            g.step(dt, NSTAGES)
-            g.max_wavespeed()
+            job.step(dt, NSTAGES)
+            job.max_wavespeed()
         barrier()
         e2e_nod2h_ms = 1e3 * (time.perf_counter() - t0)
     ms, e2e_max, e2e_nod2h_max = max_over_ranks([ms, e2e_ms or 0.0, e2e_nod2h_ms or 0.0], dist)
@@ -323,18 +336,20 @@ def main():
         return
 
     dof_per_step = pts * 9 * NSTAGES
-    value = job_value(dof_per_step, args.steps, world, ms)
+    jobs = 1 if halo else world               # halo: the ranks share ONE workload; replicas: each rank advances its own
+    value = job_value(dof_per_step, args.steps, jobs, ms)
     hbm_peak, peak_src = measured_peaks()
     main_ms, main_cnt = prof["main"]
     main_avg_ms = main_ms / max(main_cnt, 1)
+    pts_local = (job.n_owned if halo else g.E) * n ** 3      # what this GPU's kernels process per stage (roofline figures are per GPU)
     (stage_bytes, kernel_bytes), (stage_flops, kernel_flops) = alg_work(n, diff)
-    achieved = kernel_flops * pts / (main_avg_ms * 1e-3) / 1e12 if main_cnt else None        # TFLOP/s of the element kernel
+    achieved = kernel_flops * pts_local / (main_avg_ms * 1e-3) / 1e12 if main_cnt else None        # TFLOP/s of the element kernel
     kernel_ms = {k: (v[0] / max(v[1], 1)) for k, v in prof.items()}
     stage_ms = ms / (args.steps * NSTAGES)
-    t_hbm = stage_bytes * pts / (hbm_peak * 1e9) * 1e3
-    t_alu = stage_flops * pts / (FP64_PEAK_TFLOPS * 1e12) * 1e3
+    t_hbm = stage_bytes * pts_local / (hbm_peak * 1e9) * 1e3
+    t_alu = stage_flops * pts_local / (FP64_PEAK_TFLOPS * 1e12) * 1e3
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=warmup, ms_per_step=ms / args.steps,
-                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                higher_is_better=True, scaling="strong" if halo else "weak", vs_baseline=None, dtype="f64", data="synthetic",
                 config=workload_config(w, args, world, pts),
                 clocks=clocks.summary(), gpu_launches=launches,
                 roofline=dict(bound="alu", kernel="stage_main_kernel" if 4 <= n <= 7 else "residual_kernel", achieved=achieved, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
@@ -344,21 +359,21 @@ def main():
                               alg_source="model of SURVEY.md S8(d) / Appendix A5 (BASELINE.md 3), not an operation tally",
                               peak_source="nominal FP64 pipe: 148 SMs x 4 x 16 FMA/clk x 2 x 1.965 GHz (DESIGN.md 7.3)",
                               measured_fp64=peaks, alg_flops_per_point=kernel_flops, alg_bytes_per_point=kernel_bytes,
-                              kernel_hbm=dict(achieved_gbs=kernel_bytes * pts / (main_avg_ms * 1e-3) / 1e9 if main_cnt else None,
+                              kernel_hbm=dict(achieved_gbs=kernel_bytes * pts_local / (main_avg_ms * 1e-3) / 1e9 if main_cnt else None,
                                               peak_gbs=hbm_peak, peak_source=peak_src),
                               kernel_ms=kernel_ms, kernel_share_of_step={k: v[0] / prof_ms for k, v in prof.items()} if prof_ms else None,
                               kernel_timing=f"separate pass of {prof_steps} step(s) with per-launch CUDA events; the headline loop runs without them",
                               stage=dict(ms=stage_ms, alg_bytes_per_point=stage_bytes, alg_flops_per_point=stage_flops,
                                          t_hbm_ms=t_hbm, t_alu_ms=t_alu, binding="alu" if t_alu >= t_hbm else "hbm",
                                          frac_of_binding=max(t_hbm, t_alu) / stage_ms,
-                                         achieved_gbs=stage_bytes * pts / (stage_ms * 1e-3) / 1e9,
-                                         achieved_fp64_tflops=stage_flops * pts / (stage_ms * 1e-3) / 1e12)),
+                                         achieved_gbs=stage_bytes * pts_local / (stage_ms * 1e-3) / 1e9,
+                                         achieved_fp64_tflops=stage_flops * pts_local / (stage_ms * 1e-3) / 1e12)),
                 wavespeed_after=ws_after)
     if e2e_ms is not None:
-        line["e2e"] = dict(value=world * dof_per_step * e2e_steps / (e2e_ms * 1e-3), unit=UNIT, h2d_bytes_per_step=pts * 72,
-                           d2h_bytes_per_step=pts * 72 + 8, steps=e2e_steps, ms_per_step=e2e_ms / e2e_steps,
+        line["e2e"] = dict(value=jobs * dof_per_step * e2e_steps / (e2e_ms * 1e-3), unit=UNIT, h2d_bytes_per_step=int(host.numel()) * 8,
+                           d2h_bytes_per_step=int(host.numel()) * 8 + 8, steps=e2e_steps, ms_per_step=e2e_ms / e2e_steps,
                            what="chorus_set_state(pinned host) + chorus_step(dt,5) + chorus_get_state(pinned host) + chorus_max_wavespeed",
-                           without_state_d2h=dict(value=world * dof_per_step * e2e_steps / (e2e_nod2h_ms * 1e-3),
+                           without_state_d2h=dict(value=jobs * dof_per_step * e2e_steps / (e2e_nod2h_ms * 1e-3),
                                                   ms_per_step=e2e_nod2h_ms / e2e_steps, d2h_bytes_per_step=8))
     if world == 1 and not args.no_cpu_baseline:
         # the oracle on a 12,288-element sample of the same workload: one untimed residual, then one step on all cores

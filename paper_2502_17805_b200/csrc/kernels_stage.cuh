@@ -47,12 +47,18 @@ struct Mma {
   static constexpr int kTPD = (FG + kWarps - 1) / kWarps;     // directional tasks per warp and direction
   static constexpr int kTail = (3 * LO + 7) / 8;               // tail tasks per element
   static_assert(kTail <= kWarps, "tail tasks: one round");
-  // Small orders (n <= 5): an element's tiles leave room for one divergence accumulator PER DIRECTION, so no two tasks ever
-  // touch the same word: all 3 FG + kTail tasks of an element are dealt to the four chain warps with no barrier in between
-  // (n = 4: 6 tasks, n = 5: 10) instead of FG tasks per barrier-separated direction round.
+  // Orders whose tiles leave room for one divergence accumulator PER DIRECTION (n <= 5 beside a second CTA; n = 7 alone on its
+  // SM, 222 KB): no two tasks ever touch the same word, so all 3 FG + kTail tasks of an element are dealt to the chain warps
+  // with no barrier in between (n = 4: 6 tasks on 4 warps, n = 5: 10, n = 7: 19 on 8 warps) instead of FG tasks per
+  // barrier-separated direction round (at n = 7 that left two of the eight chain warps without work in every round).
+#ifdef CHORUS_DEV_NOFREE7
   static constexpr bool kFree = N <= 5;
+#else
+  static constexpr bool kFree = N <= 5 || N == 7;
+#endif
+  static constexpr int kFreeWarps = 4 * kChainWG;             // kFree: chain warps that take tasks
   static constexpr int kTasks = 3 * FG + kTail;              // kFree: tasks per element ...
-  static constexpr int kTPW = (kTasks + 3) / 4;               // ... and per chain warp
+  static constexpr int kTPW = (kTasks + kFreeWarps - 1) / kFreeWarps;   // ... and per chain warp
   // left-over lines (a,b): d = 0: b = 0, a < LO;  d = 1: b = 1, a < LO;  d = 2: a, b >= LO, the first LO of them
   __host__ __device__ static constexpr bool is_lo(int d, int ab) {
     const int a = ab % N, b = ab / N;
@@ -636,12 +642,12 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         const int g = warp + k * M::kWarps;
         lnd[d][k] = M::line_of(d, (g < M::FG ? g : 0) * 8 + L.r);
       }
-    // kFree: task i = warp + 4 t of this warp: direction, line of this thread's row, validity of the row
+    // kFree: task i = warp + kFreeWarps t of this warp: direction, line of this thread's row, validity of the row
     int fd[M::kTPW], fl[M::kTPW];
     bool fv[M::kTPW], fr[M::kTPW];        // task exists / row carries a line
 #pragma unroll
     for (int t = 0; t < M::kTPW; ++t) {
-      const int i = warp + 4 * t;
+      const int i = warp + M::kFreeWarps * t;
       fv[t] = M::kFree && i < M::kTasks;
       fr[t] = fv[t];
       fd[t] = 0; fl[t] = 0;

@@ -139,7 +139,8 @@ struct Hot {
     auto k = residual_kernel<N, DIFF, GRADV, SPILL>;
     CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 1;
-    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, smem));
+    constexpr int threads = ScalarCfg<N>::kThreads;
+    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, threads, smem));
     if (occ < 1) occ = 1;
     const int64_t cap = (int64_t)c->num_sms * occ;
     const int grid = (int)(c->E < cap ? c->E : cap);
@@ -149,7 +150,7 @@ struct Hot {
     }
     {
       ProfScope ps(c, 2);
-      k<<<grid, 256, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf[0], c->d_Vf, c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl,
+      k<<<grid, threads, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf[0], c->d_Vf, c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl,
                                          c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient, out, c->d_scratch);
     }
     ++c->launches;
@@ -249,7 +250,7 @@ struct Hot {
     auto k = grad_kernel<N, SPILL>;
     CU(c, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 1;
-    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, 256, smem));
+    CU(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k, ScalarCfg<N>::kThreads, smem));
     if (occ < 1) occ = 1;
     const int64_t cap = (int64_t)c->num_sms * occ;
     const int grid = (int)(c->E < cap ? c->E : cap);
@@ -259,7 +260,7 @@ struct Hot {
     }
     {
       ProfScope ps(c, 1);
-      k<<<grid, 256, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf[0], c->d_Sfl, c->d_jinv, c->d_krfl, c->d_nbr_elem, c->d_nbr_face,
+      k<<<grid, ScalarCfg<N>::kThreads, smem, c->stream>>>(c->E, c->ph, Qin, c->d_Qf[0], c->d_Sfl, c->d_jinv, c->d_krfl, c->d_nbr_elem, c->d_nbr_face,
                                          c->d_nbr_orient, Vf, Gout, c->d_scratch);
     }
     ++c->launches;

@@ -8,6 +8,12 @@
 
 namespace chorus {
 
+// CTA size of the scalar three-kernel path (grad_kernel, residual_kernel): orders 8 and 9 fit one CTA per SM (their tiles fill the
+// shared memory), which carries 16 warps instead of 8 to hide the latency of its shared-memory passes (measured on the sweep
+// meshes: 384 / 512 / 640 / 768 / 1024 threads give 8.6 / 8.8 / 7.5 / 6.1 / 4.7e9 DOF-updates/s at n = 8 against 7.6e9 with 256).
+template <int N> struct ScalarCfg { static constexpr int kThreads = N >= 8 ? 512 : 256; };
+
+
 // Stage the own traces and the neighbours' traces of one element in shared memory.
 //   sQo[f][v][ab] = own polynomial at the face point;  sQn[f][v][ab] = neighbour's polynomial there, or, on a
 //   wall face, the boundary state Q_b (so that "common solution" = Q_b and "outer state" = Q_b both read sQn).
@@ -91,7 +97,7 @@ __device__ __forceinline__ void br1_gradient(const ElemNbr& nb, const double* sQ
 // ---------------------------------------------------------------------------------------------------------
 // SPILL: the gradient lives in a per-CTA scratch area in global memory (n = 9: 36 n^3 doubles do not fit in shared memory)
 template <int N, bool SPILL = false>
-__global__ void __launch_bounds__(256) grad_kernel(int64_t E, PhysD ph, const double* __restrict__ Qe, const double* __restrict__ Qf,
+__global__ void __launch_bounds__(ScalarCfg<N>::kThreads) grad_kernel(int64_t E, PhysD ph, const double* __restrict__ Qe, const double* __restrict__ Qf,
                                                    const double* __restrict__ Sfl, const double* __restrict__ jinv,
                                                    const double* __restrict__ krfl, const int32_t* __restrict__ nbr_elem,
                                                    const uint8_t* __restrict__ nbr_face, const uint8_t* __restrict__ nbr_orient,

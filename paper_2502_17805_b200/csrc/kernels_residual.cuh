@@ -21,7 +21,7 @@ struct StageOut {
 // SPILL: orders whose tiles exceed the shared memory of an SM (n = 8, 9 with diffusion) keep the neighbour traces, the gradient
 // and its interpolant in a per-CTA scratch area in global memory (L2-resident: the grid is persistent) instead.
 template <int N, bool DIFF, int GRADV, bool SPILL = false>
-__global__ void __launch_bounds__(256, 1)
+__global__ void __launch_bounds__(ScalarCfg<N>::kThreads, 1)
 residual_kernel(int64_t E, PhysD ph, const double* __restrict__ Qe, const double* __restrict__ Qf, const double* __restrict__ Vf,
                 const double* __restrict__ Sfl, const double* __restrict__ detJ, const double* __restrict__ jinv,
                 const double* __restrict__ xsol, const double* __restrict__ krfl, const int32_t* __restrict__ nbr_elem,

@@ -31,6 +31,12 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
+// orders that run one CTA per SM with two chain warpgroups and free task scheduling (their tiles leave no room for a second CTA)
+__host__ __device__ constexpr bool kWideOrder(int n) { return n == 7 || n == 6; }
+// ... and, of these, the ones with room for a SECOND set of input tiles (state, own and neighbour traces, S^d): the next
+// element's inputs stream in while the current element's chains run, so the chain warps never wait for them
+__host__ __device__ constexpr bool kPrefetchOrder(int n) { return n == 6; }
+
 template <int N>
 struct Mma {
   static_assert(N >= 4 && N <= 7, "DMMA chain kernel: orders 4..7");
@@ -42,7 +48,7 @@ struct Mma {
   // would double the load of one FP64 pipe (measured: 5 warps of DMMA take twice as long as 4).
   static constexpr int FG = I::n2 / 8, LO = I::n2 % 8;
   // n = 7 leaves room for only one CTA per SM (173 KB of tiles): it gets two chain warpgroups, two chain warps per sub-partition
-  static constexpr int kChainWG = N == 7 ? 2 : 1;
+  static constexpr int kChainWG = kWideOrder(N) ? 2 : 1;
   static constexpr int kWarps = FG < 4 * kChainWG ? FG : 4 * kChainWG;
   static constexpr int kTPD = (FG + kWarps - 1) / kWarps;     // directional tasks per warp and direction
   static constexpr int kTail = (3 * LO + 7) / 8;               // tail tasks per element
@@ -51,11 +57,7 @@ struct Mma {
   // SM, 222 KB): no two tasks ever touch the same word, so all 3 FG + kTail tasks of an element are dealt to the chain warps
   // with no barrier in between (n = 4: 6 tasks on 4 warps, n = 5: 10, n = 7: 19 on 8 warps) instead of FG tasks per
   // barrier-separated direction round (at n = 7 that left two of the eight chain warps without work in every round).
-#ifdef CHORUS_DEV_NOFREE7
-  static constexpr bool kFree = N <= 5;
-#else
-  static constexpr bool kFree = N <= 5 || N == 7;
-#endif
+  static constexpr bool kFree = N <= 5 || kWideOrder(N);
   static constexpr int kFreeWarps = 4 * kChainWG;             // kFree: chain warps that take tasks
   static constexpr int kTasks = 3 * FG + kTail;              // kFree: tasks per element ...
   static constexpr int kTPW = (kTasks + kFreeWarps - 1) / kFreeWarps;   // ... and per chain warp
@@ -270,6 +272,7 @@ __device__ __forceinline__ void prefetch_block_l2(const void* p, size_t bytes, i
 // named barriers of the element kernel (id 0 is left to __syncthreads)
 enum : int { kBarChain = 1, kBarHelp = 2, kBarIn = 3, kBarGrad = 4, kBarFaces = 5, kBarRes = 6 };
 __device__ __forceinline__ void bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id, int nthreads) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 template <int R>
 __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(R)); }
 template <int R>
@@ -277,17 +280,19 @@ __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.
 
 // thread layout of the element kernel: chain warpgroup(s) first (DMMA), then one helper warpgroup (memory, faces, sources, RK)
 template <int N> struct MainCfg {
-  static constexpr int kChainWG = N == 7 ? 2 : 1;
-  static constexpr int kThreads = 128 * (kChainWG + 1);
+  static constexpr int kChainWG = kWideOrder(N) ? 2 : 1;
+  static constexpr int kHelpWG = kPrefetchOrder(N) ? 2 : 1;    // helpers that work an element ahead: twice the threads, half the latency
+  static constexpr int kThreads = 128 * (kChainWG + kHelpWG);
   static constexpr int kMinBlocks = kChainWG == 2 ? 1 : 2;
 };
 // 128 * (chain + helper) = the CTA's 256 * 128 registers: two CTAs per SM.  With diffusion the chain warps carry the streamed
 // viscous flux state and need 160; without it they are light and the helpers (sources, RK, next-state traces) get the room.
-template <bool DIFF, int CWG = 1> struct RegSplit {
-  // one chain warpgroup: launch at 128 registers (two CTAs per SM); two: launch at 168 (one CTA), 2 x 200 + 96 <= 3 x 168
-  static constexpr int kLaunch = CWG == 2 ? 168 : 128;
-  static constexpr int kChain = CWG == 2 ? 200 : DIFF ? 160 : 144;
-  static constexpr int kHelp = CWG == 2 ? 96 : 256 - kChain;
+template <bool DIFF, int CWG = 1, int HWG = 1> struct RegSplit {
+  // one chain warpgroup: launch at 128 registers (two CTAs per SM); two: launch at 168 (one CTA), 2 x 200 + 96 <= 3 x 168;
+  // two chain and two helper warpgroups (512 threads): launch at 128, 2 x 168 + 2 x 88 = 4 x 128
+  static constexpr int kLaunch = CWG == 2 ? (HWG == 2 ? 128 : 168) : 128;
+  static constexpr int kChain = CWG == 2 ? (HWG == 2 ? 168 : 200) : DIFF ? 160 : 144;     // measured at n = 6: 152 / 160 / 168 / 176 / 184
+  static constexpr int kHelp = CWG == 2 ? (HWG == 2 ? 88 : 96) : 256 - kChain;            // chain registers: 0.696 / 0.699 / 0.671 / 0.699 / 0.721 ms
 };
 
 // per-thread constants of the DMMA mapping
@@ -302,7 +307,8 @@ struct LaneK {
 
 // A3 along direction D: d Q_v / d xi_D at the solution points of 8 lines, variables GV0 .. GV0+NGV-1, into sG[(vv*3+D)]
 // D = 3: the direction is the run-time value dd (tail tasks); lv = false: the row is padding (nothing is stored)
-template <int N, int NGV, int GV0, int D>
+// COMMON: sQn already holds the common end values (BR1 average or wall state), made by the helpers' face pass an element ahead
+template <int N, int NGV, int GV0, int D, bool COMMON = false>
 __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, const double* sQ, const double* sQo, const double* sQn,
                                          double* sG, int ln, bool lv, int dd = 0) {
   using I = Ix<N>;
@@ -323,8 +329,8 @@ __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, c
       X[s] = Y[s] = sQ + sb + k * st; sX[s] = sY[s] = I::n3; wX[s] = 1.0; wY[s] = 0.0;
     } else if (k <= N + 1) {
       const int f = 2 * d + (k - N);
-      const bool wall = nb.ne[f] < 0;
-      X[s] = sQo + f * 9 * I::n2 + ln; Y[s] = sQn + f * 9 * I::n2 + ln; sX[s] = sY[s] = I::n2;
+      const bool wall = COMMON || nb.ne[f] < 0;
+      X[s] = (COMMON ? sQn : sQo) + f * 9 * I::n2 + ln; Y[s] = sQn + f * 9 * I::n2 + ln; sX[s] = sY[s] = I::n2;
       wX[s] = wall ? 0.0 : 0.5; wY[s] = wall ? 1.0 : 0.5;            // BR1 average, or the wall state
     } else {
       X[s] = Y[s] = sQ + sb; sX[s] = sY[s] = I::n3; wX[s] = 0.0; wY[s] = 0.0;   // padding: the B operand is zero
@@ -546,14 +552,21 @@ __device__ __forceinline__ void prefetch_next(const StageIO& io, const Geo& geo,
 
 // GRADV: 0 no gradient needed, 1 gradient of B only (Powell sources without diffusion), 2 all nine variables.
 //
-// One CTA = two warpgroups working on ONE element at a time:
-//   chain warps (threads 0..127, up to 4 active warps = one per SM sub-partition; 160 registers): the DMMA work -- gradient
-//     tasks, chain rule, the A1/A4/A5/A7 chains;
-//   helper warps (threads 128..255; 96 registers): everything that waits on memory or is pointwise -- cp.async of the element's
-//     inputs, wall states, the Rusanov face pass (beside the gradient), and, beside the chains, the sources and the
-//     Runge-Kutta register loads, so that after the chains only  out = w * sR + K  is left.
-// Barriers per element: IN (inputs ready) -> GRAD (gradient DMMAs done, face fluxes in registers) -> CHAINRULE (gradient and
-// face fluxes in shared memory) -> RES (divergence accumulated).
+// A CTA works on ONE element at a time with two kinds of warps:
+//   chain warps: the DMMA work -- gradient tasks, chain rule, the A1/A4/A5/A7 chains;
+//   helper warps: everything that waits on memory or is pointwise -- bulk copies of the element's inputs, wall states, the
+//     Rusanov face pass, the sources and Runge-Kutta registers (K, w), and the final combination out = w * (div_xi F~) + K.
+// Three configurations (MainCfg, RegSplit):
+//   n = 4, 5   two CTAs per SM, 4 chain warps (160 registers) + 4 helper warps (96); tasks dealt freely (kFree);
+//              barriers per element: IN (inputs ready) -> GRAD (gradient DMMAs done, face fluxes in registers) -> FACES
+//              (face fluxes in shared memory) -> RES (divergence accumulated); the helpers' face pass runs beside the gradient;
+//   n = 7      one CTA per SM (222 KB of tiles), 8 chain warps (200) + 4 helper warps (96), tasks dealt freely;
+//   n = 6      one CTA per SM, 8 chain warps (168) + 8 helper warps (88), tasks dealt freely, and TWO sets of input tiles
+//              (kPre, 218 KB in all): while the chain warps work on element e the helpers bring in element e + 1 -- bulk
+//              copies, wall states, common solution and common fluxes (face_pass) -- so the chain warps find everything
+//              ready at the IN barrier and never wait for a copy or for the Rusanov pass; the finish of element e is deferred
+//              until e + 1 has been handed over.  Barriers: IN -> FACES (accumulators free again: the helpers only arrive)
+//              -> GRAD (gradient complete: the chain warps only arrive, the helpers' sources need div B) -> RES.
 template <int N, bool DIFF, int GRADV>
 __global__ void __launch_bounds__(MainCfg<N>::kThreads, MainCfg<N>::kMinBlocks)
 stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
@@ -563,17 +576,17 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   constexpr int NGV = GRADV == 2 ? 9 : GRADV == 1 ? 3 : 0;
   constexpr int GV0 = GRADV == 1 ? 5 : 0;
   extern __shared__ __align__(16) double sm[];
-  double* sQ = sm;                       // [9][n3]
   constexpr int kOwn = 54 * I::n2 > 9 * I::n3 ? 54 * I::n2 : 9 * I::n3;
   constexpr auto ev = [](int x) { return (x + 1) & ~1; };   // keep every array 16-byte aligned
-  double* sQo = sQ + ev(9 * I::n3);      // [6][9][n2] own traces; reused as sR [9][n3] after the face pass
-  double* sQn = sQo + ev(kOwn);          // [6][9][n2] neighbour traces / wall states; overwritten by the face fluxes
-  double* sS = sQn + ev(54 * I::n2);     // [3 fam][3 comp][nf] S^d at the flux points (cp.async; 9*nf is even)
-  double* sG = sS + 9 * I::nf;           // [3*NGV][n3]
-  double* sR = sQo;
+  // one set of INPUT tiles: sQ [9][n3] | sQo [6][9][n2] own traces, reused as sR [9][n3] after the face pass | sQn [6][9][n2]
+  // neighbour traces / wall states, overwritten by the face fluxes | sS [3 fam][3 comp][nf] S^d at the flux points
+  constexpr int kIn = ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + 9 * I::nf;
+  constexpr bool kPre = kPrefetchOrder(N);   // two input sets, used alternately (element i of this CTA: set i & 1)
+  double* sG = sm + (kPre ? 2 : 1) * kIn;    // [3*NGV][n3]
   double* sR12 = sG + ev(3 * NGV * I::n3);   // kFree: the accumulators of directions 1 and 2, [2][9][n3] (direction 0: sR)
   constexpr int kRS = ev(9 * I::n3);
-  __shared__ ElemNbr nb;
+  double* sR0 = sR12 + 2 * kRS;              // kPre: direction 0 has its own accumulator too (sQo holds the face fluxes then)
+  __shared__ ElemNbr nbs[2];
   __shared__ int s_second;
   __shared__ __align__(8) uint64_t mbar;   // completion of the bulk (TMA) copies of one element
   if (threadIdx.x == 0) {
@@ -585,13 +598,13 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   }
   __syncthreads();
   constexpr int kMainThreads = MainCfg<N>::kThreads, kCT = 128 * M::kChainWG;      // all threads / chain threads
-  using RS = RegSplit<DIFF, M::kChainWG>;
+  using RS = RegSplit<DIFF, M::kChainWG, MainCfg<N>::kHelpWG>;
   const bool is_chain = M::kChainWG == 1 ? (threadIdx.x >> 7) == 0 : threadIdx.x < kCT;
   const int tid = M::kChainWG == 1 ? (int)(threadIdx.x & 127) : is_chain ? (int)threadIdx.x : (int)threadIdx.x - kCT;
   // The contiguous per-element blocks (state, own traces, S^d) go by TMA bulk copy when they are 16-byte aligned (n even);
   // the neighbour traces are gathered through the orientation map with 8-byte cp.async either way.
   constexpr bool kBulk = (9 * I::n3) % 2 == 0 && (54 * I::n2) % 2 == 0;
-  constexpr int H = 128;                 // helper threads
+  constexpr int H = 128 * MainCfg<N>::kHelpWG;   // helper threads
 
   if (is_chain) {
     // =============================================== chain warps ===============================================
@@ -668,7 +681,16 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     int tail_rot = s_second ? M::kWarps / 2 : 0;
     constexpr int P2 = (I::n3 + CH - 1) / CH;     // solution points per chain thread in the chain rule
     unsigned ld_phase = 0;
-    for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
+    int it = 0;
+    for (int64_t e = blockIdx.x; e < E; e += gridDim.x, ++it) {
+      const int cur = kPre ? (it & 1) : 0;
+      double* sQ = sm + cur * kIn;
+      double* sQo = sQ + ev(9 * I::n3);
+      double* sQn = sQo + ev(kOwn);
+      double* sS = sQn + ev(54 * I::n2);
+      double* sR = kPre ? sR0 : sQo;
+      double* sFace = kPre ? sQo : sQn;       // where the common face fluxes are
+      const ElemNbr& nb = nbs[cur];
       int tw = M::kWarps, tl_d = 0, tl_ln = 0;
       bool tl_ok = false;
       if (M::kTail > 0 && active) {
@@ -699,7 +721,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       if constexpr (GRADV != 0 && M::kFree) {
 #pragma unroll
         for (int t = 0; t < M::kTPW; ++t)
-          if (fv[t]) grad_dir<N, NGV, GV0, 3>(L, nb, sQ, sQo, sQn, sG, fl[t], fr[t], fd[t]);
+          if (fv[t]) grad_dir<N, NGV, GV0, 3, kPre>(L, nb, sQ, sQo, sQn, sG, fl[t], fr[t], fd[t]);
       } else if constexpr (GRADV != 0) {
         if (active) {
 #pragma unroll
@@ -712,7 +734,11 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           if (M::kTail > 0 && tw < M::kTail) grad_dir<N, NGV, GV0, 3>(L, nb, sQ, sQo, sQn, sG, tl_ln, tl_ok, tl_d);
         }
       }
-      bar_sync(kBarGrad, kMainThreads);        // gradient DMMAs done (the helpers hold the face fluxes in registers)
+      // gradient DMMAs done: the helpers, who hold the first face fluxes in registers, may overwrite the neighbour traces.  The
+      // chain warps only signal it (the chain rule and the first interpolations need nothing from the Rusanov pass) and
+      // synchronise among themselves: the chain rule mixes the three directions' derivatives of every warp.
+      if (!kPre) bar_arrive(kBarGrad, kMainThreads);
+      bar_sync(kBarChain, CH);
       if constexpr (GRADV != 0) {
 #pragma unroll
         for (int q = 0; q < P2; ++q) {
@@ -728,14 +754,15 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         }
       }
       bar_sync(kBarChain, CH);                  // the gradient is complete in shared memory
+      if (kPre) bar_arrive(kBarGrad, kMainThreads);   // ... which the helpers' sources (div B) wait for
       if constexpr (M::kFree) {
         // ---- A1, A4, A5, A7: every task stores into the accumulator of its own direction; no barrier between tasks
 #pragma unroll
         for (int t = 0; t < M::kTPW; ++t) {
           if (!fv[t]) continue;
           double* acc = fd[t] == 0 ? sR : sR12 + (fd[t] - 1) * kRS;
-          if (t == 0) chain_dir<N, DIFF, 3, true, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, acc, fl[t], fr[t], fd[t], tid);
-          else chain_dir<N, DIFF, 3, false, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, acc, fl[t], fr[t], fd[t]);
+          if (t == 0) chain_dir<N, DIFF, 3, true, 1>(L, ph, nb, io, geo, e, sQ, sG, sFace, sS, acc, fl[t], fr[t], fd[t], tid);
+          else chain_dir<N, DIFF, 3, false, 1>(L, ph, nb, io, geo, e, sQ, sG, sFace, sS, acc, fl[t], fr[t], fd[t]);
         }
       } else {
       // ---- A1, A4, A5, A7: one DMMA chain per warp and direction, directions separated by chain-warp barriers
@@ -795,7 +822,11 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     // asynchronous load of one element's inputs: state, own traces, S^d, neighbour traces through the orientation map (A2)
     // part A: state, S^d and neighbour traces (their shared memory is dead as soon as the chains are done);
     // part B: own traces (their region doubles as the divergence accumulator sR, read by the final combination)
-    auto issue_loads_a = [&](int64_t el) {
+    auto issue_loads_a = [&](int64_t el, int set) {
+      double* sQ = sm + set * kIn;
+      double* sQn = sQ + ev(9 * I::n3) + ev(kOwn);
+      double* sS = sQn + ev(54 * I::n2);
+      ElemNbr& nb = nbs[set];
       if (tid < 6) { nb.ne[tid] = pn_e; nb.nf[tid] = pn_f; nb.no[tid] = pn_o; }
       const double* q = io.Qe + el * 9 * I::n3;
       const double* g = geo.Sfl + el * 9 * I::nf;
@@ -833,7 +864,8 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         }
       }
     };
-    auto issue_loads_b = [&](int64_t el) {
+    auto issue_loads_b = [&](int64_t el, int set) {
+      double* sQo = sm + set * kIn + ev(9 * I::n3);
       const double* t = io.Qf + el * 54 * I::n2;
       if (kBulk) {
         if (tid == 64) {
@@ -848,15 +880,171 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     };
     fetch_nbr(blockIdx.x);
     if ((int64_t)blockIdx.x < E) {
-      issue_loads_a(blockIdx.x);
-      issue_loads_b(blockIdx.x);
+      issue_loads_a(blockIdx.x, 0);
+      issue_loads_b(blockIdx.x, 0);
       fetch_nbr((int64_t)blockIdx.x + gridDim.x);
     }
     const bool rk = io.Qout != nullptr;
     const bool g0 = rk && io.A0 != nullptr, g1 = rk && io.A1 != nullptr;
 
+    double K[P2][9], w[P2];                     // sources and Runge-Kutta registers of this thread's points (set beside the chains)
+    auto finish = [&](int64_t ef, int setf) {   // out = w * (div_xi F~) + K for element ef, whose tiles are input set setf
+      double* sQ = sm + setf * kIn;
+      double* sR = kPre ? sR0 : sQ + ev(9 * I::n3);
+#pragma unroll
+      for (int q = 0; q < P2; ++q) {
+        const int s = tid + q * H;
+        if (s < I::n3) {
+          double R[9];
+#pragma unroll
+          for (int v = 0; v < 9; ++v) {
+            double dv = sR[v * I::n3 + s];
+            if (M::kFree) dv += sR12[v * I::n3 + s] + sR12[kRS + v * I::n3 + s];     // one accumulator per direction
+            R[v] = w[q] * dv + K[q][v];
+          }
+          if (DIFF) {                    // finished by the face kernel
+#pragma unroll
+            for (int v = 0; v < 9; ++v) io.Part[(ef * 9 + v) * I::n3 + s] = R[v];
+          } else if (rk) {
+#pragma unroll
+            for (int v = 0; v < 9; ++v) {
+              io.Qout[(ef * 9 + v) * I::n3 + s] = R[v];
+              sQ[v * I::n3 + s] = R[v];   // this thread is the only reader and writer of point s in this phase
+            }
+          } else {
+#pragma unroll
+            for (int v = 0; v < 9; ++v) io.Rout[((int64_t)v * E + ef) * I::n3 + s] = R[v];
+          }
+        }
+      }
+      if (!DIFF && rk) {
+        bar_sync(kBarHelp, H);
+        emit_traces<N>(sQ, io.QfOut + ef * 54 * I::n2, tid, H);
+      }
+      bar_sync(kBarHelp, H);                   // every helper is done with this element's shared memory
+    };
+    // A8 sources and the Runge-Kutta registers of element es (state tile sQ), so that  out = w * (div_xi F~) + K  is all that is left
+    auto sources = [&](int64_t e, const double* sQ) {
+#pragma unroll
+      for (int q = 0; q < P2; ++q) {
+        const int s = tid + q * H;
+        const int sc = s < I::n3 ? s : 0;
+        double Q[9];
+#pragma unroll
+        for (int v = 0; v < 9; ++v) Q[v] = sQ[v * I::n3 + sc];
+        double divB = 0.0;
+        if (GRADV == 2) divB = sG[15 * I::n3 + sc] + sG[19 * I::n3 + sc] + sG[23 * I::n3 + sc];
+        if (GRADV == 1) divB = sG[0 * I::n3 + sc] + sG[4 * I::n3 + sc] + sG[8 * I::n3 + sc];
+        {
+          const PrimD p = primitives(ph, Q);
+#pragma unroll
+          for (int v = 0; v < 9; ++v) K[q][v] = 0.0;
+          add_sources(ph, p, divB, geo.xsol[(e * 3 + 0) * I::n3 + sc], geo.xsol[(e * 3 + 1) * I::n3 + sc],
+                      geo.xsol[(e * 3 + 2) * I::n3 + sc], K[q]);                                      // K = M (Eq. 5)
+        }
+        w[q] = -1.0 / geo.detJ[e * I::n3 + sc];              // R = w * div_xi F~ + M  (Eq. 16)
+        if (rk) {                                            // step mode: out = cq Q + c0 A0 + c1 A1 + bdt R
+          w[q] *= io.bdt;
+#pragma unroll
+          for (int v = 0; v < 9; ++v) K[q][v] = io.bdt * K[q][v] + io.cq * Q[v];
+          if (g0) {
+#pragma unroll
+            for (int v = 0; v < 9; ++v) K[q][v] += io.c0 * io.A0[(e * 9 + v) * I::n3 + sc];
+          }
+          if (g1) {
+#pragma unroll
+            for (int v = 0; v < 9; ++v) K[q][v] += io.c1 * io.A1[(e * 9 + v) * I::n3 + sc];
+          }
+        }
+      }
+    };
+    // kPre: walls and common inviscid fluxes of element el (input set `set`) an element ahead: the common SOLUTION (BR1 average
+    // or wall state Q_b) replaces the neighbour traces, the common FLUX (Rusanov / wall, scaled by sigma |S|) the own traces
+    auto face_pass = [&](int64_t el, int set) {
+      double* sQo = sm + set * kIn + ev(9 * I::n3);
+      double* sQn = sQo + ev(kOwn);
+      const ElemNbr& nb = nbs[set];
+      for (int t = tid; t < 6 * I::n2; t += H) {
+        const int f = t / I::n2, ab = t % I::n2;
+        const double* nf_ = geo.nfc + (el * 6 + f) * 4 * I::n2 + ab;
+        const double nx = nf_[0], ny = nf_[I::n2], nz = nf_[2 * I::n2], sa = nf_[3 * I::n2];
+        double Qi[9], Qc[9], F[9];
+#pragma unroll
+        for (int v = 0; v < 9; ++v) Qi[v] = sQo[(f * 9 + v) * I::n2 + ab];
+        if (nb.ne[f] >= 0) {
+          double Qo[9];
+#pragma unroll
+          for (int v = 0; v < 9; ++v) Qo[v] = sQn[(f * 9 + v) * I::n2 + ab];
+          flux_rusanov(ph, Qi, Qo, nx, ny, nz, F);
+#pragma unroll
+          for (int v = 0; v < 9; ++v) Qc[v] = 0.5 * Qi[v] + 0.5 * Qo[v];          // BR1
+        } else {
+          wall_state(ph, nb.ne[f], Qi, nx, ny, nz, Qc);
+          const PrimD sb_ = primitives(ph, Qc);
+          flux_inviscid<true>(ph, sb_, nx, ny, nz, F);
+        }
+#pragma unroll
+        for (int v = 0; v < 9; ++v) {
+          sQn[(f * 9 + v) * I::n2 + ab] = Qc[v];
+          sQo[(f * 9 + v) * I::n2 + ab] = sa * F[v];
+        }
+      }
+    };
     unsigned ld_phase = 0;
-    for (int64_t e = blockIdx.x; e < E; e += gridDim.x) {
+    int it = 0;
+    int64_t e_last = -1;
+    if constexpr (kPre) {
+      // ---- two input sets: everything the chain warps need of element e -- inputs, wall states, common fluxes -- is made
+      //      while they work on element e - 1; the finish of e - 1 happens after e has been handed over
+      if ((int64_t)blockIdx.x < E) {
+        cp_async_wait_all();
+        mbar_wait(&mbar, ld_phase);
+        ld_phase ^= 1u;
+        bar_sync(kBarHelp, H);
+        face_pass(blockIdx.x, 0);
+      }
+      for (int64_t e = blockIdx.x; e < E; e += gridDim.x, ++it) {
+        const int cur = it & 1;
+        const bool more = e + gridDim.x < E;
+        e_last = e;
+        bar_sync(kBarIn, kMainThreads);              // inputs, common solution and common fluxes of e are in shared memory
+        // With diffusion the finish of the previous element touches no input tile (it writes Part from the accumulators): the
+        // next loads go first, so that the proxy fence of their issuing threads does not wait for the finish's global stores.
+        if (DIFF && more) {
+          issue_loads_a(e + gridDim.x, cur ^ 1);
+          issue_loads_b(e + gridDim.x, cur ^ 1);
+          fetch_nbr(e + 2 * (int64_t)gridDim.x);
+        }
+        if (it > 0) finish(e - gridDim.x, cur ^ 1);  // previous element: reads the accumulators, frees its input set
+        bar_arrive(kBarFaces, kMainThreads);         // the accumulators are free for this element's chains
+        if (!DIFF && more) {
+          issue_loads_a(e + gridDim.x, cur ^ 1);
+          issue_loads_b(e + gridDim.x, cur ^ 1);
+          fetch_nbr(e + 2 * (int64_t)gridDim.x);
+        }
+        if (e + 2 * (int64_t)gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + 2 * (int64_t)gridDim.x, pn_e, pn_f, tid, H);
+        if (more) {
+          cp_async_wait_all();
+          mbar_wait(&mbar, ld_phase);
+          ld_phase ^= 1u;
+          bar_sync(kBarHelp, H);
+          face_pass(e + gridDim.x, cur ^ 1);
+        }
+        bar_sync(kBarGrad, kMainThreads);            // the gradient of e is complete (div B of the Powell sources)
+        sources(e, sm + cur * kIn);
+        bar_sync(kBarRes, kMainThreads);
+      }
+      if (e_last >= 0) finish(e_last, (it - 1) & 1);
+    } else
+
+    for (int64_t e = blockIdx.x; e < E; e += gridDim.x, ++it) {
+      const int cur = kPre ? (it & 1) : 0;
+      double* sQ = sm + cur * kIn;
+      double* sQo = sQ + ev(9 * I::n3);
+      double* sQn = sQo + ev(kOwn);
+      e_last = e;
+      const ElemNbr& nb = nbs[cur];
+      const bool more = e + gridDim.x < E;
       cp_async_wait_all();
       if (kBulk) mbar_wait(&mbar, ld_phase);   // the bulk copies have landed ...
       ld_phase ^= 1u;
@@ -916,86 +1104,25 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       }
       bar_sync(kBarFaces, kMainThreads);
 
-      // ---- beside the chains: A8 sources and the Runge-Kutta registers, so that  out = w * sR + K  is all that is left
-      double K[P2][9], w[P2];
-#pragma unroll
-      for (int q = 0; q < P2; ++q) {
-        const int s = tid + q * H;
-        const int sc = s < I::n3 ? s : 0;
-        double Q[9];
-#pragma unroll
-        for (int v = 0; v < 9; ++v) Q[v] = sQ[v * I::n3 + sc];
-        double divB = 0.0;
-        if (GRADV == 2) divB = sG[15 * I::n3 + sc] + sG[19 * I::n3 + sc] + sG[23 * I::n3 + sc];
-        if (GRADV == 1) divB = sG[0 * I::n3 + sc] + sG[4 * I::n3 + sc] + sG[8 * I::n3 + sc];
-        {
-          const PrimD p = primitives(ph, Q);
-#pragma unroll
-          for (int v = 0; v < 9; ++v) K[q][v] = 0.0;
-          add_sources(ph, p, divB, geo.xsol[(e * 3 + 0) * I::n3 + sc], geo.xsol[(e * 3 + 1) * I::n3 + sc],
-                      geo.xsol[(e * 3 + 2) * I::n3 + sc], K[q]);                                      // K = M (Eq. 5)
-        }
-        w[q] = -1.0 / geo.detJ[e * I::n3 + sc];              // R = w * div_xi F~ + M  (Eq. 16)
-        if (rk) {                                            // step mode: out = cq Q + c0 A0 + c1 A1 + bdt R
-          w[q] *= io.bdt;
-#pragma unroll
-          for (int v = 0; v < 9; ++v) K[q][v] = io.bdt * K[q][v] + io.cq * Q[v];
-          if (g0) {
-#pragma unroll
-            for (int v = 0; v < 9; ++v) K[q][v] += io.c0 * io.A0[(e * 9 + v) * I::n3 + sc];
-          }
-          if (g1) {
-#pragma unroll
-            for (int v = 0; v < 9; ++v) K[q][v] += io.c1 * io.A1[(e * 9 + v) * I::n3 + sc];
-          }
-        }
-      }
+      sources(e, sQ);                          // beside the chains
       // measured: -0.9k cycles of the 6.2k the chain warps wait for the next element's inputs
-      if (e + gridDim.x < E) prefetch_next<N, GRADV>(io, geo, e + gridDim.x, pn_e, pn_f, tid, H);
+      if (e + (kPre ? 2 : 1) * (int64_t)gridDim.x < E)
+        prefetch_next<N, GRADV>(io, geo, e + (kPre ? 2 : 1) * (int64_t)gridDim.x, pn_e, pn_f, tid, H);
       bar_sync(kBarRes, kMainThreads);
 
       // ---- A9: finish the element.  The next element's state, metrics and neighbour traces start streaming in first
-      //      (except when this element's new state still has to pass through sQ for its traces)
+      //      (except when this element's new state still has to pass through sQ for its traces).  With two input sets the
+      //      finish is deferred until the NEXT element's inputs have been handed to the chain warps (top of the loop).
       constexpr bool kEarlyLoads = DIFF;
-      const bool more = e + gridDim.x < E;
-      if (kEarlyLoads && more) issue_loads_a(e + gridDim.x);
-#pragma unroll
-      for (int q = 0; q < P2; ++q) {
-        const int s = tid + q * H;
-        if (s < I::n3) {
-          double R[9];
-#pragma unroll
-          for (int v = 0; v < 9; ++v) {
-            double dv = sR[v * I::n3 + s];
-            if (M::kFree) dv += sR12[v * I::n3 + s] + sR12[kRS + v * I::n3 + s];     // one accumulator per direction
-            R[v] = w[q] * dv + K[q][v];
-          }
-          if (DIFF) {                    // finished by the face kernel
-#pragma unroll
-            for (int v = 0; v < 9; ++v) io.Part[(e * 9 + v) * I::n3 + s] = R[v];
-          } else if (rk) {
-#pragma unroll
-            for (int v = 0; v < 9; ++v) {
-              io.Qout[(e * 9 + v) * I::n3 + s] = R[v];
-              sQ[v * I::n3 + s] = R[v];   // this thread is the only reader and writer of point s in this phase
-            }
-          } else {
-#pragma unroll
-            for (int v = 0; v < 9; ++v) io.Rout[((int64_t)v * E + e) * I::n3 + s] = R[v];
-          }
-        }
-      }
-      if (!DIFF && rk) {
-        bar_sync(kBarHelp, H);
-        emit_traces<N>(sQ, io.QfOut + e * 54 * I::n2, tid, H);
-      }
-      bar_sync(kBarHelp, H);                   // every helper is done with this element's shared memory
-      if (more) {
-        if (!kEarlyLoads) issue_loads_a(e + gridDim.x);
-        issue_loads_b(e + gridDim.x);
+      if (!kPre && kEarlyLoads && more) issue_loads_a(e + gridDim.x, 0);
+      if (!kPre) finish(e, 0);
+      if (!kPre && more) {
+        if (!kEarlyLoads) issue_loads_a(e + gridDim.x, 0);
+        issue_loads_b(e + gridDim.x, 0);
         fetch_nbr(e + 2 * (int64_t)gridDim.x);
       }
     }
+
   }
 }
 
@@ -1005,8 +1132,8 @@ constexpr size_t stage_main_smem_bytes() {
   constexpr int NGV = GRADV == 2 ? 9 : GRADV == 1 ? 3 : 0;
   constexpr int kOwn = 54 * I::n2 > 9 * I::n3 ? 54 * I::n2 : 9 * I::n3;
   constexpr auto ev = [](int x) { return (x + 1) & ~1; };
-  return sizeof(double) * (size_t)(ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + 9 * I::nf + ev(3 * NGV * I::n3) +
-                                   (Mma<N>::kFree ? 2 * ev(9 * I::n3) : 0));
+  return sizeof(double) * (size_t)((kPrefetchOrder(N) ? 2 : 1) * (ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + 9 * I::nf) +
+                                   ev(3 * NGV * I::n3) + (Mma<N>::kFree ? (kPrefetchOrder(N) ? 3 : 2) * ev(9 * I::n3) : 0));
 }
 
 // ---------------------------------------------------------------------------------------------------------

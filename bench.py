@@ -352,7 +352,7 @@ def main():
                 higher_is_better=True, scaling="strong" if halo else "weak", vs_baseline=None, dtype="f64", data="synthetic",
                 config=workload_config(w, args, world, pts),
                 clocks=clocks.summary(), gpu_launches=launches,
-                roofline=dict(bound="alu", kernel="stage_main_kernel" if 4 <= n <= 7 else "residual_kernel", achieved=achieved, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
+                roofline=dict(bound="alu", kernel="stage_main_kernel" if 4 <= n <= 8 else "residual_kernel", achieved=achieved, peak=FP64_PEAK_TFLOPS, unit="TFLOP/s",
                               frac=(achieved / FP64_PEAK_TFLOPS) if achieved else None, traffic=ncu_traffic(args.workload),
                               traffic_source="dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu --set full "
                                              "capture (profiles/roofline_traffic.md); not measured in this run",

@@ -63,7 +63,7 @@ struct chorus_ctx {
   double* d_scratch = nullptr;      // per-CTA global scratch of the scalar kernels' SPILL variants (orders 8, 9 with diffusion)
   size_t scratch_doubles = 0;
   int64_t launches = 0;
-  bool use_mma = true;   // orders 4..7: two-kernel DMMA pipeline (kernels_stage.cuh); CHORUS_KERNELS=scalar selects the
+  bool use_mma = true;   // orders 4..8: two-kernel DMMA pipeline (kernels_stage.cuh); CHORUS_KERNELS=scalar selects the
                          // three-kernel shared-memory path that serves the other orders (kernels_residual.cuh)
   bool prof = false;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[3];
@@ -162,10 +162,10 @@ struct Hot {
     if (residual_smem_bytes<N, DIFF, GRADV, false>() <= c->max_smem) return residual_launch_impl<DIFF, GRADV, false>(c, Qin, out);
     return residual_launch_impl<DIFF, GRADV, true>(c, Qin, out);
   }
-  // ---- production pipeline (orders 4..7): main kernel, then (diffusion) the face kernel
+  // ---- production pipeline (orders 4..8): main kernel, then (diffusion) the face kernel
   template <bool DIFF, int GRADV>
   static int main_launch(chorus_ctx* c, const StageIO& io) {
-    if constexpr (N >= 4 && N <= 7) {
+    if constexpr (kMmaOrder(N)) {
       constexpr size_t smem = stage_main_smem_bytes<N, GRADV>();
       constexpr int threads = MainCfg<N>::kThreads;
       auto k = stage_main_kernel<N, DIFF, GRADV>;
@@ -184,7 +184,7 @@ struct Hot {
       CU(c, cudaGetLastError());
       return CHORUS_OK;
     } else {
-      return fail(c, CHORUS_EINVAL, "the DMMA pipeline serves orders 4..7");
+      return fail(c, CHORUS_EINVAL, "the DMMA pipeline serves orders 4..8");
     }
   }
   static int face_launch(chorus_ctx* c, const StageIO& io) {
@@ -292,7 +292,7 @@ struct Hot {
   // finishes it (chorus_stage_face).  A partition exchanges halo data between the two.
   static int face_pending(chorus_ctx* c) { return stage_pipeline_face(c, c->pend); }
   static int ensure_traces(chorus_ctx* c, const double* Qin) {
-    if (!(c->use_mma && N >= 4 && N <= 7)) return fail(c, CHORUS_EINVAL, "the split step serves the DMMA pipeline (orders 4..7)");
+    if (!(c->use_mma && kMmaOrder(N))) return fail(c, CHORUS_EINVAL, "the split step serves the DMMA pipeline (orders 4..8)");
     if (!c->traces_valid) {
       int rc = trace(c, Qin, c->d_Qf[c->qf_cur]);
       if (rc) return rc;
@@ -301,7 +301,7 @@ struct Hot {
     return CHORUS_OK;
   }
   static int stage(chorus_ctx* c, const double* Qin, const StageOut& out, double* scratch, bool split = false) {
-    if (!(c->use_mma && N >= 4 && N <= 7)) return split ? fail(c, CHORUS_EINVAL, "the split step serves orders 4..7") : stage_legacy(c, Qin, out);
+    if (!(c->use_mma && kMmaOrder(N))) return split ? fail(c, CHORUS_EINVAL, "the split step serves orders 4..8") : stage_legacy(c, Qin, out);
     if (!c->traces_valid) {
       int rc = trace(c, Qin, c->d_Qf[c->qf_cur]);
       if (rc) return rc;

@@ -1,4 +1,4 @@
-// kernels_stage.cuh -- the production pipeline of one residual evaluation / Runge-Kutta stage (orders 4..7).
+// kernels_stage.cuh -- the production pipeline of one residual evaluation / Runge-Kutta stage (orders 4..8).
 //
 //   stage_main_kernel  per element: A2 face gather + BR1 common solution, A3 gradient (computed ONCE per stage),
 //                      A6 Rusanov / wall inviscid face fluxes, A1 + A4 + A5 + A7 as register-resident FP64 tensor-core
@@ -31,15 +31,22 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
-// orders that run one CTA per SM with two chain warpgroups and free task scheduling (their tiles leave no room for a second CTA)
-__host__ __device__ constexpr bool kWideOrder(int n) { return n == 7 || n == 6; }
+// orders served by this pipeline
+__host__ __device__ constexpr bool kMmaOrder(int n) { return n >= 4 && n <= 8; }
+// orders that run one CTA per SM with two chain warpgroups (their tiles leave no room for a second CTA)
+__host__ __device__ constexpr bool kWideOrder(int n) { return n >= 6 && n <= 8; }
+// n = 8: the n + 1 = 9 flux points of a line do not fit the 8 columns of a DMMA tile.  The tile holds the 7 interior flux points
+// and the face point m = n; the face point m = 0 enters the flux derivative as a third k-step whose A operand is the common face
+// flux in shared memory, and the own-side viscous flux of the three m = 0 faces (Vf) is made by the helper warps.  S^d is read
+// from global memory (L2) instead of a shared-memory tile: 212 KB of tiles in all.
+__host__ __device__ constexpr bool kFaceOutOrder(int n) { return n == 8; }
 // ... and, of these, the ones with room for a SECOND set of input tiles (state, own and neighbour traces, S^d): the next
 // element's inputs stream in while the current element's chains run, so the chain warps never wait for them
 __host__ __device__ constexpr bool kPrefetchOrder(int n) { return n == 6; }
 
 template <int N>
 struct Mma {
-  static_assert(N >= 4 && N <= 7, "DMMA chain kernel: orders 4..7");
+  static_assert(kMmaOrder(N), "DMMA chain kernel: orders 4..8");
   using I = Ix<N>;
   // Lines of a direction are handed to warps in groups of 8 (the M dimension of the DMMA).  n^2 = 8 FG + LO: the FG full
   // groups of a direction are "directional tasks" (compile-time direction); the LO left-over lines of the three directions
@@ -57,7 +64,7 @@ struct Mma {
   // SM, 222 KB): no two tasks ever touch the same word, so all 3 FG + kTail tasks of an element are dealt to the chain warps
   // with no barrier in between (n = 4: 6 tasks on 4 warps, n = 5: 10, n = 7: 19 on 8 warps) instead of FG tasks per
   // barrier-separated direction round (at n = 7 that left two of the eight chain warps without work in every round).
-  static constexpr bool kFree = N <= 5 || kWideOrder(N);
+  static constexpr bool kFree = N <= 7;                      // n = 8: one accumulator, barrier-separated direction rounds of 8 tasks
   static constexpr int kFreeWarps = 4 * kChainWG;             // kFree: chain warps that take tasks
   static constexpr int kTasks = 3 * FG + kTail;              // kFree: tasks per element ...
   static constexpr int kTPW = (kTasks + kFreeWarps - 1) / kFreeWarps;   // ... and per chain warp
@@ -85,8 +92,8 @@ struct Mma {
   // pass serves both (cols 2c+1 of the last two thread columns that hold anything).
   __device__ __forceinline__ static int col_m(int j) {
     // 4 bits per column, value m + 1 (0 = padding).  N = 4: {1,2,3,0,-,4,-,-}; 5: {1,2,3,4,-,0,-,5}; 6: {1,2,3,4,5,0,-,6};
-    // 7: {1,2,3,4,5,0,6,7}
-    constexpr uint32_t tbl = N == 4 ? 0x00501432u : N == 5 ? 0x60105432u : N == 6 ? 0x70165432u : 0x87165432u;
+    // 7: {1,2,3,4,5,0,6,7}; 8: {1,2,3,4,5,6,7,8} (the face point m = 0 is not in the tile: kFaceOutOrder)
+    constexpr uint32_t tbl = N == 4 ? 0x00501432u : N == 5 ? 0x60105432u : N == 6 ? 0x70165432u : N == 7 ? 0x87165432u : 0x98765432u;
     return (int)((tbl >> (4 * j)) & 15u) - 1;
   }
 };
@@ -281,7 +288,8 @@ __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.
 // thread layout of the element kernel: chain warpgroup(s) first (DMMA), then one helper warpgroup (memory, faces, sources, RK)
 template <int N> struct MainCfg {
   static constexpr int kChainWG = kWideOrder(N) ? 2 : 1;
-  static constexpr int kHelpWG = kPrefetchOrder(N) ? 2 : 1;    // helpers that work an element ahead: twice the threads, half the latency
+  // helpers that work an element ahead: twice the threads, half the latency; n = 8: 512 points and the face viscous fluxes
+  static constexpr int kHelpWG = kPrefetchOrder(N) || kFaceOutOrder(N) ? 2 : 1;
   static constexpr int kThreads = 128 * (kChainWG + kHelpWG);
   static constexpr int kMinBlocks = kChainWG == 2 ? 1 : 2;
 };
@@ -300,6 +308,7 @@ template <int N>
 struct LaneK {
   double bI0, bI1;     // interpolation operand, k-steps 0 and 1
   double bD0, bD1;     // derivative operand
+  double bD2;          // kFaceOutOrder: derivative operand of the third k-step (k = 0: face point m = 0; k >= 1: zero)
   double bG[3];        // BR1 gradient operand
   int m0, m1;          // flux point of the two columns this thread holds (-1 = padding)
   int r, c;
@@ -339,7 +348,7 @@ __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, c
   const double* A0 = sQ + sb + c * st;          // k-step 0: k = c < N
   const bool ok0 = lv && 2 * c < N, ok1 = lv && 2 * c + 1 < N;
   double* out = sG + d * I::n3 + sb + (2 * c) * st;
-  constexpr int VB = NGV % 3 == 0 ? 3 : 1;      // variables in flight (hides the DMMA latency)
+  constexpr int VB = NGV % 3 == 0 ? 3 : 1;      // variables in flight (hides the DMMA latency; 9 at a time measured slower)
 #pragma unroll
   for (int v0 = 0; v0 < NGV; v0 += VB) {
     double d0[VB], d1[VB];
@@ -521,6 +530,11 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
   for (int v = 0; v < 9; ++v) dmma884z(r0[v], r1[v], q0[v], L.bD0);
 #pragma unroll
   for (int v = 0; v < 9; ++v) dmma884(r0[v], r1[v], q1[v], L.bD1);
+  if constexpr (kFaceOutOrder(N)) {   // third k-step: the common flux of the line's face point m = 0 (k = 0; the B operand of k >= 1 is zero)
+    const double* f = sFace + ((2 * d) * 9) * I::n2 + ln;
+#pragma unroll
+    for (int v = 0; v < 9; ++v) dmma884(r0[v], r1[v], f[v * I::n2], L.bD2);
+  }
   if (SYNCB) bar_sync(kBarChain, 128 * Mma<N>::kChainWG);     // every update of the previous round is in sR
 #pragma unroll
   for (int v = 0; v < 9; ++v) {
@@ -580,7 +594,8 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   constexpr auto ev = [](int x) { return (x + 1) & ~1; };   // keep every array 16-byte aligned
   // one set of INPUT tiles: sQ [9][n3] | sQo [6][9][n2] own traces, reused as sR [9][n3] after the face pass | sQn [6][9][n2]
   // neighbour traces / wall states, overwritten by the face fluxes | sS [3 fam][3 comp][nf] S^d at the flux points
-  constexpr int kIn = ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + 9 * I::nf;
+  constexpr bool kSglobal = kFaceOutOrder(N);   // S^d read from global memory by the chains (no shared-memory tile)
+  constexpr int kIn = ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + (kSglobal ? 0 : 9 * I::nf);
   constexpr bool kPre = kPrefetchOrder(N);   // two input sets, used alternately (element i of this CTA: set i & 1)
   double* sG = sm + (kPre ? 2 : 1) * kIn;    // [3*NGV][n3]
   double* sR12 = sG + ev(3 * NGV * I::n3);   // kFree: the accumulators of directions 1 and 2, [2][9][n3] (direction 0: sR)
@@ -633,6 +648,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         if (L.m0 >= 0) L.bD0 = op.Dfs[r * (N + 1) + L.m0];
         if (L.m1 >= 0) L.bD1 = op.Dfs[r * (N + 1) + L.m1];
       }
+      L.bD2 = (r < N && c == 0) ? op.Dfs[r * (N + 1)] : 0.0;
       // BR1 gradient: x = (q_0..q_{N-1}, common value at m = 0, at m = N), K = N + 2 -> up to 3 k-steps of 4
       // B[k][n = l_out r]: k < N: Dss[l_out][k]; k = N: Dfs[l_out][0]; k = N+1: Dfs[l_out][N]
 #pragma unroll
@@ -687,7 +703,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       double* sQ = sm + cur * kIn;
       double* sQo = sQ + ev(9 * I::n3);
       double* sQn = sQo + ev(kOwn);
-      double* sS = sQn + ev(54 * I::n2);
+      const double* sS = kSglobal ? geo.Sfl + e * 9 * I::nf : sQn + ev(54 * I::n2);
       double* sR = kPre ? sR0 : sQo;
       double* sFace = kPre ? sQo : sQn;       // where the common face fluxes are
       const ElemNbr& nb = nbs[cur];
@@ -838,20 +854,21 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           const unsigned cnt = __popc(__ballot_sync(0xffffffffu, whole));
           if (tid == 0) {
             fence_proxy_async();
-            mbar_expect_tx(&mbar, (unsigned)(sizeof(double) * (9 * I::n3 + 9 * I::nf + cnt * 9 * I::n2)));
+            mbar_expect_tx(&mbar, (unsigned)(sizeof(double) * (9 * I::n3 + (kSglobal ? 0 : 9 * I::nf) + cnt * 9 * I::n2)));
             tma_load(sQ, q, sizeof(double) * 9 * I::n3, &mbar);
           }
           if (whole) {
             if (tid != 0) fence_proxy_async();
             tma_load(sQn + tid * 9 * I::n2, io.Qf + ((int64_t)pn_e * 6 + pn_f) * 9 * I::n2, sizeof(double) * 9 * I::n2, &mbar);
           }
-        } else if (tid == 32) {
+        } else if (tid == 32 && !kSglobal) {
           fence_proxy_async();
           tma_load(sS, g, sizeof(double) * 9 * I::nf, &mbar);
         }
       } else {
         for (int k = tid; k < 9 * I::n3; k += H) cp_async8(sQ + k, q + k);
-        for (int k = tid; k < 9 * I::nf / 2; k += H) cp_async16(sS + 2 * k, g + 2 * k);
+        if (!kSglobal)
+          for (int k = tid; k < 9 * I::nf / 2; k += H) cp_async16(sS + 2 * k, g + 2 * k);
       }
       bar_sync(kBarHelp, H);   // nb visible
       for (int k = tid; k < 6 * I::n2; k += H) {
@@ -1104,6 +1121,70 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       }
       bar_sync(kBarFaces, kMainThreads);
 
+      if constexpr (DIFF && kFaceOutOrder(N)) {
+        // Own-side viscous flux at the 3 n^2 points of the faces m = 0 (not in the chains' tiles): Q and grad Q interpolated to the
+        // face point (Eq. 19), evaluated on Q_in (interior face) or on the wall state Q_b, along the outward unit normal.  The
+        // gradient is complete: the chain warps reached FACES after their chain rule.
+        const OpsC& op = c_ops[N];
+        for (int t = tid; t < 3 * I::n2; t += H) {
+          const int d = t / I::n2, ab = t % I::n2, f = 2 * d;
+          const int st = I::stride(d), sb = I::sbase(d, ab);
+          // The lines of a warp's 32 face points start 8 or 64 doubles apart: read in the same order they would meet in two
+          // (direction 0) or eight (direction 1) shared-memory banks.  Each lane walks its line from its own starting point
+          // instead (l = (j + rot) mod 8), which spreads a half-warp over all 32 banks.
+          static_assert(N == 8, "bank rotation written for n = 8");
+          const int rot = d == 0 ? ((((ab & 7) >> 1) + 4 * ((ab >> 3) & 1)) & 7) : d == 1 ? ((ab >> 3) & 1) : 0;
+          double wI[N];
+          int lo[N];
+#pragma unroll
+          for (int j = 0; j < N; ++j) {
+            const int l = (j + rot) & 7;
+            wI[j] = op.Isf[((f & 1) ? N * N : 0) + l];
+            lo[j] = sb + l * st;
+          }
+          double q[9];
+#pragma unroll
+          for (int v = 0; v < 9; ++v) {
+            double a = 0.0;
+#pragma unroll
+            for (int j = 0; j < N; ++j) a += wI[j] * sQ[v * I::n3 + lo[j]];
+            q[v] = a;
+          }
+          const double* nf_ = geo.nfc + ((e * 6 + f) * 4) * I::n2 + ab;
+          const double nx = nf_[0], ny = nf_[I::n2], nz = nf_[2 * I::n2];
+          const int ne = nb.ne[f];
+          if (ne < 0) {
+            double qb[9];
+            wall_state(ph, ne, q, nx, ny, nz, qb);
+#pragma unroll
+            for (int v = 0; v < 9; ++v) q[v] = qb[v];
+          }
+          const PrimD p = primitives(ph, q);
+          VStream vs;
+#define CHORUS_FACE_VAR(V)                                                              \
+  {                                                                                     \
+    double g0 = 0.0, g1 = 0.0, g2 = 0.0;                                                \
+    const double* G = sG + (3 * (V)) * I::n3;                                           \
+    _Pragma("unroll") for (int j = 0; j < N; ++j) {                                     \
+      const double wl = wI[j];                                                          \
+      g0 += wl * G[lo[j]];                                                              \
+      g1 += wl * G[I::n3 + lo[j]];                                                      \
+      g2 += wl * G[2 * I::n3 + lo[j]];                                                  \
+    }                                                                                   \
+    vs_fold<V>(vs, p, nx, ny, nz, g0, g1, g2);                                          \
+  }
+          CHORUS_FACE_VAR(0) CHORUS_FACE_VAR(1) CHORUS_FACE_VAR(2) CHORUS_FACE_VAR(3) CHORUS_FACE_VAR(4)
+          CHORUS_FACE_VAR(5) CHORUS_FACE_VAR(6) CHORUS_FACE_VAR(7) CHORUS_FACE_VAR(8)
+#undef CHORUS_FACE_VAR
+          const double kr = geo.krfl ? geo.krfl[(e * 3 + d) * I::nf + I::fbase(d, ab) + ((f & 1) ? N : 0) * st] : 0.0;
+          double Fv[7];
+          if (ne < 0) vs_flux_wall(ph, ne, vs, p, nx, ny, nz, kr, Fv);
+          else vs_flux(ph, vs, p, nx, ny, nz, kr, Fv);
+          double* o = io.Vf + ((e * 6 + f) * 7) * I::n2 + ab;
+#pragma unroll
+          for (int k = 0; k < 7; ++k) o[k * I::n2] = Fv[k];
+        }
+      }
       sources(e, sQ);                          // beside the chains
       // measured: -0.9k cycles of the 6.2k the chain warps wait for the next element's inputs
       if (e + (kPre ? 2 : 1) * (int64_t)gridDim.x < E)
@@ -1132,7 +1213,7 @@ constexpr size_t stage_main_smem_bytes() {
   constexpr int NGV = GRADV == 2 ? 9 : GRADV == 1 ? 3 : 0;
   constexpr int kOwn = 54 * I::n2 > 9 * I::n3 ? 54 * I::n2 : 9 * I::n3;
   constexpr auto ev = [](int x) { return (x + 1) & ~1; };
-  return sizeof(double) * (size_t)((kPrefetchOrder(N) ? 2 : 1) * (ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + 9 * I::nf) +
+  return sizeof(double) * (size_t)((kPrefetchOrder(N) ? 2 : 1) * (ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + (kFaceOutOrder(N) ? 0 : 9 * I::nf)) +
                                    ev(3 * NGV * I::n3) + (Mma<N>::kFree ? (kPrefetchOrder(N) ? 3 : 2) * ev(9 * I::n3) : 0));
 }
 

@@ -168,7 +168,7 @@ def test_order_sweep_parity(n, diff):
     assert g25_error(g.get_state(), o.get_state(), phys.c_h).max() <= STATE_TOL
 
 
-@pytest.mark.parametrize("n,diff", [(4, 1e-3), (4, 0.0), (5, 1e-3), (5, 0.0), (6, 1e-3), (6, 0.0), (7, 1e-3), (7, 0.0)])
+@pytest.mark.parametrize("n,diff", [(4, 1e-3), (4, 0.0), (5, 1e-3), (5, 0.0), (6, 1e-3), (6, 0.0), (7, 1e-3), (7, 0.0), (8, 1e-3), (8, 0.0)])
 def test_persistent_loop_parity(n, diff):
     """Meshes with more elements (6x8x8x2 = 768) than the element kernel's grid (2 CTAs x 148 SMs, 1 x 148 at n = 7), so that
     every CTA runs its persistent loop several times -- barrier phases, bulk copies into live shared memory, tail-task rotation,
@@ -244,7 +244,7 @@ def test_empty_and_single_element_edge_cases():
         P.Chorus(empty, 3, phys)
 
 
-@pytest.mark.parametrize("n,diff", [(6, 1e-3), (6, 0.0), (5, 1e-3), (4, 1e-3), (7, 1e-3)])
+@pytest.mark.parametrize("n,diff", [(6, 1e-3), (6, 0.0), (5, 1e-3), (4, 1e-3), (7, 1e-3), (8, 1e-3)])
 def test_bitwise_reproducible_across_launches(n, diff):
     """The element kernel is warp-specialised (chain and helper warps hand shared memory to each other through named
     barriers) and has no atomics on its data path: repeated launches must agree bit for bit.  A missing barrier shows up
@@ -366,3 +366,37 @@ def test_flux_balanced_background_with_radiative_profile_parity():
     o.set_physics(phys)
     r1, _ = o.residual(True)
     assert g24_error(r1, r0, a0).max() > 1e-6
+
+
+@pytest.mark.parametrize("wall_opts", [dict(bc_mag_inner=I.BC_RADIAL, bc_mag_outer=I.BC_CONDUCTING, kr_scale=2e-3, kr_c=(1.0, -0.5, 0.25),
+                                            kr_wscale=1.3, T_top=0.05, q_bottom=0.02,
+                                            extra_flags=I.FLAG_FIXED_T_OUTER | I.FLAG_FIXED_FLUX_INNER | I.FLAG_CENTRIFUGAL),
+                                       dict(bc_mag_inner=I.BC_CONDUCTING, bc_mag_outer=I.BC_RADIAL)])
+def test_order8_walls_and_orientations_parity(wall_opts):
+    """n = 8 on the DMMA pipeline: its tiles hold the interior flux points and the face point m = n; the face point m = 0 goes
+    through the helper warps (own-side viscous flux) and a third k-step (flux derivative).  Both wall types on both walls with
+    the thermal options and kappa_r(r), and every face orientation of a scrambled box with diffusion."""
+    kw = dict(wall_opts)
+    extra = kw.pop("extra_flags", 0)
+    w, mesh, o, g, Q, phys = shell_case(8, 3, 2, 3.0, 7, 2e-3, u_amp=0.01, b_amp=0.05, extra_flags=extra, **kw)
+    check_residual(o, g)
+    _, xf, _, _ = P.get_operators(8)
+    dt = w.dt(o.max_wavespeed(), xf[1] - xf[0])
+    for _ in range(2):
+        o.step(dt, 5); g.step(dt, 5)
+    assert g25_error(g.get_state(), o.get_state(), phys.c_h).max() <= STATE_TOL
+    n = 8
+    mesh = I.scrambled_box(2, 2, 3, (1.0, 1.1, 0.9), I.lobatto_abscissae(n + 1), seed=8, distort=0.1)
+    physb = I.Physics(c_h=1.2, nu=0.01, kappa=0.02, eta=0.015, flags=I.FLAG_POWELL | I.FLAG_DIFFUSION)
+    o, g = ob.Oracle(mesh, n, physb), P.Chorus(mesh, n, physb)
+    x = o.geometry()["xsol"]
+    rng = np.random.default_rng(3)
+    sh = x.shape[1:]
+    Q = I.conserved(1 + 0.2 * np.sin(3 * x[0]) + 0.05 * rng.uniform(-1, 1, sh), 0.2 * rng.uniform(-1, 1, (3,) + sh) + 0.1,
+                    1 + 0.1 * np.cos(2 * x[1]), 0.3 * rng.uniform(-1, 1, (3,) + sh) + 0.2, 0.1 * rng.uniform(-1, 1, sh), 5 / 3)
+    o.set_state(Q); g.set_state(Q)
+    check_residual(o, g)
+    Q[:] = I.conserved(1.2, np.zeros(3), 1.5, np.zeros(3), np.float64(0.0), 5 / 3)[:, None, None]
+    o.set_state(Q); g.set_state(Q)
+    _, a = o.residual(True)
+    assert np.abs(g.residual()).max() <= 1e-13 * a.max()

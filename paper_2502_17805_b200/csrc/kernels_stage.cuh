@@ -40,6 +40,12 @@ __host__ __device__ constexpr bool kWideOrder(int n) { return n >= 6 && n <= 8; 
 // flux in shared memory, and the own-side viscous flux of the three m = 0 faces (Vf) is made by the helper warps.  S^d is read
 // from global memory (L2) instead of a shared-memory tile: 212 KB of tiles in all.
 __host__ __device__ constexpr bool kFaceOutOrder(int n) { return n == 8; }
+// orders whose chains read S^d at the flux points from global memory (L2; prefetched an element ahead) instead of a shared-memory tile
+#ifndef CHORUS_DEV_SGLOBAL6
+__host__ __device__ constexpr bool kSglobalOrder(int n) { return n == 8; }
+#else
+__host__ __device__ constexpr bool kSglobalOrder(int n) { return n == 8 || n == 6; }
+#endif
 // ... and, of these, the ones with room for a SECOND set of input tiles (state, own and neighbour traces, S^d): the next
 // element's inputs stream in while the current element's chains run, so the chain warps never wait for them
 __host__ __device__ constexpr bool kPrefetchOrder(int n) { return n == 6; }
@@ -288,19 +294,22 @@ __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.
 // thread layout of the element kernel: chain warpgroup(s) first (DMMA), then one helper warpgroup (memory, faces, sources, RK)
 template <int N> struct MainCfg {
   static constexpr int kChainWG = kWideOrder(N) ? 2 : 1;
-  // helpers that work an element ahead: twice the threads, half the latency; n = 8: 512 points and the face viscous fluxes
-  static constexpr int kHelpWG = kPrefetchOrder(N) || kFaceOutOrder(N) ? 2 : 1;
+  // one CTA per SM: two helper warpgroups as well.  The helpers' phases (wall states, Rusanov pass, sources, final combination,
+  // loads) are latency-bound and partly in series with the chains: twice the threads, half the time (n = 7 measured with one
+  // helper warpgroup at 96 registers and 200-register chains: 4.17 ms on sweep_n7; with two at 88 and 168-register chains: 3.40)
+  static constexpr int kHelpWG = kWideOrder(N) ? 2 : 1;
   static constexpr int kThreads = 128 * (kChainWG + kHelpWG);
   static constexpr int kMinBlocks = kChainWG == 2 ? 1 : 2;
 };
 // 128 * (chain + helper) = the CTA's 256 * 128 registers: two CTAs per SM.  With diffusion the chain warps carry the streamed
 // viscous flux state and need 160; without it they are light and the helpers (sources, RK, next-state traces) get the room.
 template <bool DIFF, int CWG = 1, int HWG = 1> struct RegSplit {
-  // one chain warpgroup: launch at 128 registers (two CTAs per SM); two: launch at 168 (one CTA), 2 x 200 + 96 <= 3 x 168;
-  // two chain and two helper warpgroups (512 threads): launch at 128, 2 x 168 + 2 x 88 = 4 x 128
-  static constexpr int kLaunch = CWG == 2 ? (HWG == 2 ? 128 : 168) : 128;
-  static constexpr int kChain = CWG == 2 ? (HWG == 2 ? 168 : 200) : DIFF ? 160 : 144;     // measured at n = 6: 152 / 160 / 168 / 176 / 184
-  static constexpr int kHelp = CWG == 2 ? (HWG == 2 ? 88 : 96) : 256 - kChain;            // chain registers: 0.696 / 0.699 / 0.671 / 0.699 / 0.721 ms
+  // one chain warpgroup: launch at 128 registers (two CTAs per SM);
+  // two chain and two helper warpgroups (512 threads, one CTA per SM): launch at 128, 2 x 168 + 2 x 88 = 4 x 128
+  static_assert(CWG == HWG, "one chain + one helper warpgroup, or two + two");
+  static constexpr int kLaunch = 128;
+  static constexpr int kChain = CWG == 2 ? 168 : DIFF ? 160 : 144;     // measured at n = 6: 152 / 160 / 168 / 176 / 184
+  static constexpr int kHelp = CWG == 2 ? 88 : 256 - kChain;           // chain registers: 0.696 / 0.699 / 0.671 / 0.699 / 0.721 ms
 };
 
 // per-thread constants of the DMMA mapping
@@ -390,6 +399,19 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
   const int l1 = 4 + c < N ? 4 + c : N - 1;     // second k-step: l = 4 + c, clamped where the B operand is zero anyway
   const double* A0 = sQ + sb + c * st;
   const double* A1 = sQ + sb + l1 * st;
+  const bool int0 = m0 > 0 && m0 < N, int1 = m1 > 0 && m1 < N;
+  const int fb = I::fbase(d, ln);
+  double S0x = 0.0, S0y = 0.0, S0z = 0.0, S1x = 0.0, S1y = 0.0, S1z = 0.0, kr0 = 0.0, kr1 = 0.0;
+  if constexpr (kSglobalOrder(N)) {   // S^d comes from global memory (L2): issued first, needed after the first interpolations
+    if (int0) {
+      const double* s = sS + (d * 3) * I::nf + fb + m0 * st;
+      S0x = s[0]; S0y = s[I::nf]; S0z = s[2 * I::nf];
+    }
+    if (int1) {
+      const double* s = sS + (d * 3) * I::nf + fb + m1 * st;
+      S1x = s[0]; S1y = s[I::nf]; S1z = s[2 * I::nf];
+    }
+  }
   // A1: Q at the two flux points of this thread
   double q0[9], q1[9];
 #pragma unroll
@@ -399,16 +421,13 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
     for (int v = 0; v < 9; ++v) dmma884(q0[v], q1[v], A1[v * I::n3], L.bI1);
   }
   // per-slot setup: area vector and the state the fluxes are evaluated on
-  const bool int0 = m0 > 0 && m0 < N, int1 = m1 > 0 && m1 < N;
   const bool face0 = m0 == 0 || m0 == N, face1 = m1 == 0 || m1 == N;     // m = -1: padding
-  const int fb = I::fbase(d, ln);
-  double S0x = 0.0, S0y = 0.0, S0z = 0.0, S1x = 0.0, S1y = 0.0, S1z = 0.0, kr0 = 0.0, kr1 = 0.0;
   int fc0 = 0, fc1 = 0;
-  if (int0) {
+  if (!kSglobalOrder(N) && int0) {
     const double* s = sS + (d * 3) * I::nf + fb + m0 * st;
     S0x = s[0]; S0y = s[I::nf]; S0z = s[2 * I::nf];
   }
-  if (int1) {
+  if (!kSglobalOrder(N) && int1) {
     const double* s = sS + (d * 3) * I::nf + fb + m1 * st;
     S1x = s[0]; S1y = s[I::nf]; S1z = s[2 * I::nf];
   }
@@ -570,11 +589,13 @@ __device__ __forceinline__ void prefetch_next(const StageIO& io, const Geo& geo,
 //   chain warps: the DMMA work -- gradient tasks, chain rule, the A1/A4/A5/A7 chains;
 //   helper warps: everything that waits on memory or is pointwise -- bulk copies of the element's inputs, wall states, the
 //     Rusanov face pass, the sources and Runge-Kutta registers (K, w), and the final combination out = w * (div_xi F~) + K.
-// Three configurations (MainCfg, RegSplit):
+// Four configurations (MainCfg, RegSplit):
 //   n = 4, 5   two CTAs per SM, 4 chain warps (160 registers) + 4 helper warps (96); tasks dealt freely (kFree);
 //              barriers per element: IN (inputs ready) -> GRAD (gradient DMMAs done, face fluxes in registers) -> FACES
 //              (face fluxes in shared memory) -> RES (divergence accumulated); the helpers' face pass runs beside the gradient;
-//   n = 7      one CTA per SM (222 KB of tiles), 8 chain warps (200) + 4 helper warps (96), tasks dealt freely;
+//   n = 7      one CTA per SM (222 KB of tiles), 8 chain warps (168) + 8 helper warps (88), tasks dealt freely;
+//   n = 8      one CTA per SM (212 KB), 8 + 8 warps, three barrier-separated direction rounds of 8 tasks on one accumulator;
+//              its tiles hold 7 interior flux points and the face point m = n (kFaceOutOrder), S^d comes from L2;
 //   n = 6      one CTA per SM, 8 chain warps (168) + 8 helper warps (88), tasks dealt freely, and TWO sets of input tiles
 //              (kPre, 218 KB in all): while the chain warps work on element e the helpers bring in element e + 1 -- bulk
 //              copies, wall states, common solution and common fluxes (face_pass) -- so the chain warps find everything
@@ -594,7 +615,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   constexpr auto ev = [](int x) { return (x + 1) & ~1; };   // keep every array 16-byte aligned
   // one set of INPUT tiles: sQ [9][n3] | sQo [6][9][n2] own traces, reused as sR [9][n3] after the face pass | sQn [6][9][n2]
   // neighbour traces / wall states, overwritten by the face fluxes | sS [3 fam][3 comp][nf] S^d at the flux points
-  constexpr bool kSglobal = kFaceOutOrder(N);   // S^d read from global memory by the chains (no shared-memory tile)
+  constexpr bool kSglobal = kSglobalOrder(N);   // S^d read from global memory by the chains (no shared-memory tile)
   constexpr int kIn = ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + (kSglobal ? 0 : 9 * I::nf);
   constexpr bool kPre = kPrefetchOrder(N);   // two input sets, used alternately (element i of this CTA: set i & 1)
   double* sG = sm + (kPre ? 2 : 1) * kIn;    // [3*NGV][n3]
@@ -1213,7 +1234,7 @@ constexpr size_t stage_main_smem_bytes() {
   constexpr int NGV = GRADV == 2 ? 9 : GRADV == 1 ? 3 : 0;
   constexpr int kOwn = 54 * I::n2 > 9 * I::n3 ? 54 * I::n2 : 9 * I::n3;
   constexpr auto ev = [](int x) { return (x + 1) & ~1; };
-  return sizeof(double) * (size_t)((kPrefetchOrder(N) ? 2 : 1) * (ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + (kFaceOutOrder(N) ? 0 : 9 * I::nf)) +
+  return sizeof(double) * (size_t)((kPrefetchOrder(N) ? 2 : 1) * (ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + (kSglobalOrder(N) ? 0 : 9 * I::nf)) +
                                    ev(3 * NGV * I::n3) + (Mma<N>::kFree ? (kPrefetchOrder(N) ? 3 : 2) * ev(9 * I::n3) : 0));
 }
 

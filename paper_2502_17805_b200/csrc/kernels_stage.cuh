@@ -41,11 +41,7 @@ __host__ __device__ constexpr bool kWideOrder(int n) { return n >= 6 && n <= 8; 
 // from global memory (L2) instead of a shared-memory tile: 212 KB of tiles in all.
 __host__ __device__ constexpr bool kFaceOutOrder(int n) { return n == 8; }
 // orders whose chains read S^d at the flux points from global memory (L2; prefetched an element ahead) instead of a shared-memory tile
-#ifndef CHORUS_DEV_SGLOBAL6
-__host__ __device__ constexpr bool kSglobalOrder(int n) { return n == 8; }
-#else
 __host__ __device__ constexpr bool kSglobalOrder(int n) { return n == 8 || n == 6; }
-#endif
 // ... and, of these, the ones with room for a SECOND set of input tiles (state, own and neighbour traces, S^d): the next
 // element's inputs stream in while the current element's chains run, so the chain warps never wait for them
 __host__ __device__ constexpr bool kPrefetchOrder(int n) { return n == 6; }
@@ -283,7 +279,7 @@ __device__ __forceinline__ void prefetch_block_l2(const void* p, size_t bytes, i
 }
 
 // named barriers of the element kernel (id 0 is left to __syncthreads)
-enum : int { kBarChain = 1, kBarHelp = 2, kBarIn = 3, kBarGrad = 4, kBarFaces = 5, kBarRes = 6 };
+enum : int { kBarChain = 1, kBarHelp = 2, kBarIn = 3, kBarGrad = 4, kBarFaces = 5, kBarRes = 6, kBarNext = 7, kBarWave = 8 };
 __device__ __forceinline__ void bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 __device__ __forceinline__ void bar_arrive(int id, int nthreads) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 template <int R>
@@ -385,9 +381,10 @@ __device__ __forceinline__ void grad_dir(const LaneK<N>& L, const ElemNbr& nb, c
 // chain rule and the first interpolations) are awaited here, just before they are needed, and the left-over direction-0
 // points of sR are zeroed.
 // STORE: 1 store the divergence contribution, 0 accumulate it, -1 (default): store for direction 0, accumulate otherwise.
-// SYNCB: this is the warp's first task of a round that accumulates: the chain-warp barrier that separates the rounds is taken
-// here, just before the update, instead of before the task (the warps drift apart by less than the barrier used to cost).
-template <int N, bool DIFF, int D, bool WAITF = false, int STORE = -1, bool SYNCB = false>
+// SYNCB: 1: this is the warp's first task of a round that accumulates: the chain-warp barrier that separates the rounds is taken
+// here, just before the update, instead of before the task (the warps drift apart by less than the barrier used to cost);
+// 2: the same with the barrier between the two waves of the kPre pipeline (the warps without a second task only arrive).
+template <int N, bool DIFF, int D, bool WAITF = false, int STORE = -1, int SYNCB = 0>
 __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, const ElemNbr& nb, const StageIO& io, const Geo& geo,
                                           int64_t e, const double* sQ, const double* sG, const double* sFace, const double* sS, double* sR,
                                           int ln, bool lv, int dd = 0, int ctid = 0) {
@@ -554,7 +551,8 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
 #pragma unroll
     for (int v = 0; v < 9; ++v) dmma884(r0[v], r1[v], f[v * I::n2], L.bD2);
   }
-  if (SYNCB) bar_sync(kBarChain, 128 * Mma<N>::kChainWG);     // every update of the previous round is in sR
+  if (SYNCB == 1) bar_sync(kBarChain, 128 * Mma<N>::kChainWG);     // every update of the previous round is in sR
+  if (SYNCB == 2) bar_sync(kBarWave, 128 * Mma<N>::kChainWG);      // kPre: every store of the first wave is in the accumulators
 #pragma unroll
   for (int v = 0; v < 9; ++v) {
     constexpr bool kStore = STORE == 1 || (STORE == -1 && D == 0);
@@ -596,12 +594,14 @@ __device__ __forceinline__ void prefetch_next(const StageIO& io, const Geo& geo,
 //   n = 7      one CTA per SM (222 KB of tiles), 8 chain warps (168) + 8 helper warps (88), tasks dealt freely;
 //   n = 8      one CTA per SM (212 KB), 8 + 8 warps, three barrier-separated direction rounds of 8 tasks on one accumulator;
 //              its tiles hold 7 interior flux points and the face point m = n (kFaceOutOrder), S^d comes from L2;
-//   n = 6      one CTA per SM, 8 chain warps (168) + 8 helper warps (88), tasks dealt freely, and TWO sets of input tiles
-//              (kPre, 218 KB in all): while the chain warps work on element e the helpers bring in element e + 1 -- bulk
-//              copies, wall states, common solution and common fluxes (face_pass) -- so the chain warps find everything
-//              ready at the IN barrier and never wait for a copy or for the Rusanov pass; the finish of element e is deferred
-//              until e + 1 has been handed over.  Barriers: IN -> FACES (accumulators free again: the helpers only arrive)
-//              -> GRAD (gradient complete: the chain warps only arrive, the helpers' sources need div B) -> RES.
+//   n = 6      one CTA per SM, 8 chain warps (168) + 8 helper warps (88), TWO sets of input tiles and TWO gradient buffers
+//              (kPre, 213 KB in all; S^d from L2): while the chain warps work on element e the helpers bring in element
+//              e + 1 -- bulk copies, wall states, common solution and common fluxes (face_pass) -- and the two chain warps
+//              that have no task in the element's second wave compute the gradient of e + 1, so that between two elements
+//              only the chain rule is left; the finish of element e is deferred until e + 1 is under way.  Barriers per
+//              element: FACES (accumulators free: helpers arrive, chains wait inside their first task) -> WAVE (first-wave
+//              stores done; chains only) -> NEXT (inputs of e + 1 handed over: helpers arrive, the gradient warps wait) ->
+//              RES (chains done with e: they only arrive) -> GRAD (gradient of e + 1 complete: chains only arrive).
 template <int N, bool DIFF, int GRADV>
 __global__ void __launch_bounds__(MainCfg<N>::kThreads, MainCfg<N>::kMinBlocks)
 stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
@@ -618,12 +618,13 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   constexpr bool kSglobal = kSglobalOrder(N);   // S^d read from global memory by the chains (no shared-memory tile)
   constexpr int kIn = ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + (kSglobal ? 0 : 9 * I::nf);
   constexpr bool kPre = kPrefetchOrder(N);   // two input sets, used alternately (element i of this CTA: set i & 1)
-  double* sG = sm + (kPre ? 2 : 1) * kIn;    // [3*NGV][n3]
-  double* sR12 = sG + ev(3 * NGV * I::n3);   // kFree: the accumulators of directions 1 and 2, [2][9][n3] (direction 0: sR)
-  constexpr int kRS = ev(9 * I::n3);
-  double* sR0 = sR12 + 2 * kRS;              // kPre: direction 0 has its own accumulator too (sQo holds the face fluxes then)
+  double* sG = sm + (kPre ? 2 : 1) * kIn;    // [3*NGV][n3]; kPre: two of them (the gradient of the next element is made ahead)
+  constexpr int kGS = ev(3 * NGV * I::n3);
+  double* sR12 = sG + (kPre ? 2 : 1) * kGS;  // kFree: the accumulators of directions 1 and 2, [2][9][n3] (direction 0: sR);
+  constexpr int kRS = ev(9 * I::n3);         // kPre: the two accumulators of the two task waves (see the chain loop)
   __shared__ ElemNbr nbs[2];
   __shared__ int s_second;
+  __shared__ int s_task[kPre ? M::kTasks * 8 : 1];   // kPre: (task, row) -> line | direction << 16 | row carries a line << 20
   __shared__ __align__(8) uint64_t mbar;   // completion of the bulk (TMA) copies of one element
   if (threadIdx.x == 0) {
     unsigned smid;
@@ -631,6 +632,22 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     s_second = (int)(atomicAdd(io.sm_arrivals + smid, 1u) & 1u);
     mbar_init(&mbar, 2);     // two producer arrivals per element: part A and part B of its loads
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  if constexpr (kPre) {
+    for (int t = threadIdx.x; t < M::kTasks * 8; t += blockDim.x) {
+      const int i = t >> 3, r = t & 7;
+      int d, ln, ok = 1;
+      if (i < 3 * M::FG) {
+        d = i / M::FG;
+        ln = M::line_of(d, (i % M::FG) * 8 + r);
+      } else {
+        const int q = (i - 3 * M::FG) * 8 + r;               // index among the 3 LO left-over lines
+        ok = q < 3 * M::LO;
+        d = ok ? q / (M::LO > 0 ? M::LO : 1) : 0;
+        ln = M::line_of(d, 8 * M::FG + (ok ? q % (M::LO > 0 ? M::LO : 1) : 0));
+      }
+      s_task[t] = ln | (d << 16) | (ok << 20);
+    }
   }
   __syncthreads();
   constexpr int kMainThreads = MainCfg<N>::kThreads, kCT = 128 * M::kChainWG;      // all threads / chain threads
@@ -719,14 +736,125 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     constexpr int P2 = (I::n3 + CH - 1) / CH;     // solution points per chain thread in the chain rule
     unsigned ld_phase = 0;
     int it = 0;
+    if constexpr (kPre) {
+      // ---- The pipeline of the order with two sets of input tiles and two gradient buffers.  An element's 14 tasks run in two
+      //      waves on the 8 chain warps: wave 1 = the 2 FG full-group tasks of directions 0 and 1 (one per warp; each STORES
+      //      into the accumulator of its direction, acc0 / acc1), wave 2 = the FG tasks of direction 2 (warps 0..FG-1, which ADD
+      //      into acc0) and the tail tasks (which ADD into acc1; left-over lines never meet in a point).  The warps without a
+      //      second task (kGW0..7) compute the NEXT element's gradient tasks meanwhile, into the other gradient buffer, so that
+      //      the gradient phase leaves the critical path: between two elements only the chain rule is left.
+      static_assert(M::kTPW == 2 && 2 * M::FG == M::kFreeWarps && M::kChainWG == 2, "wave structure of the kPre pipeline");
+      constexpr int kGW0 = M::kTasks - M::kFreeWarps;          // first warp without a second-wave task
+      constexpr int kGW = M::kFreeWarps - kGW0;                // warps that make the next gradient
+      double* acc0 = sR12;
+      double* acc1 = sR12 + kRS;
+      auto wait_inputs = [&]() {                               // bulk copies: completion is observed by every consumer thread itself
+        if (kBulk) mbar_wait(&mbar, ld_phase);
+        ld_phase ^= 1u;
+      };
+      double jv[P2][9];
+      auto load_jv = [&](int64_t el) {     // chain-rule metrics of this thread's solution points (L2-resident: prefetched ahead)
+        if (GRADV != 0) {
+#pragma unroll
+          for (int q = 0; q < P2; ++q) {
+            const int sc = tid + q * CH < I::n3 ? tid + q * CH : 0;
+#pragma unroll
+            for (int k = 0; k < 9; ++k) jv[q][k] = geo.jinv[el * 9 * I::n3 + k * I::n3 + sc];
+          }
+        }
+      };
+      auto chain_rule = [&](double* G) {
+        if constexpr (GRADV != 0) {
+#pragma unroll
+          for (int q = 0; q < P2; ++q) {
+            const int sp = tid + q * CH;
+            if (sp < I::n3) {
+#pragma unroll
+              for (int vv = 0; vv < NGV; ++vv) {
+                const double g0 = G[(vv * 3 + 0) * I::n3 + sp], g1 = G[(vv * 3 + 1) * I::n3 + sp], g2 = G[(vv * 3 + 2) * I::n3 + sp];
+#pragma unroll
+                for (int pp = 0; pp < 3; ++pp) G[(vv * 3 + pp) * I::n3 + sp] = jv[q][pp] * g0 + jv[q][3 + pp] * g1 + jv[q][6 + pp] * g2;
+              }
+            }
+          }
+        }
+      };
+      // first element: its gradient is made by all chain warps
+      if ((int64_t)blockIdx.x < E) {
+        load_jv(blockIdx.x);
+        wait_inputs();
+        bar_sync(kBarIn, kMainThreads);          // inputs, common solution and common fluxes of the first element are in shared memory
+        if constexpr (GRADV != 0) {
+          const double* q0 = sm;
+#pragma unroll
+          for (int t = 0; t < M::kTPW; ++t)
+            if (fv[t]) grad_dir<N, NGV, GV0, 3, true>(L, nbs[0], q0, q0 + ev(9 * I::n3), q0 + ev(9 * I::n3) + ev(kOwn), sG, fl[t], fr[t], fd[t]);
+        }
+        bar_sync(kBarChain, CH);
+        chain_rule(sG);
+        bar_sync(kBarChain, CH);
+        bar_arrive(kBarGrad, kMainThreads);      // the gradient is complete: the helpers' sources (div B) wait for it
+      }
+      for (int64_t e = blockIdx.x; e < E; e += gridDim.x, ++it) {
+        const int cur = it & 1;
+        const bool more = e + gridDim.x < E;
+        double* sQ = sm + cur * kIn;
+        double* sQo = sQ + ev(9 * I::n3);        // the common face fluxes
+        const double* sS = geo.Sfl + e * 9 * I::nf;
+        const double* sGc = sG + cur * kGS;
+        // wave 1: stores; the FACES barrier (accumulators free) is taken inside, just before the common fluxes are needed
+        chain_dir<N, DIFF, 3, true, 1>(L, ph, nbs[cur], io, geo, e, sQ, sGc, sQo, sS, fd[0] == 0 ? acc0 : acc1, fl[0], fr[0], fd[0], tid);
+        // the points of the left-over lines of directions 0 and 1, which no first-wave task stores, start from zero
+        if constexpr (M::LO > 0) {
+          for (int t = tid; t < 2 * 9 * M::LO * N; t += CH) {
+            const int l = t % N, i = (t / N) % M::LO, v = (t / (N * M::LO)) % 9, d = t / (9 * N * M::LO);
+            const int ln = s_task[(3 * M::FG) * 8 + d * M::LO + i] & 0xffff;      // tail rows: direction-major, LO lines each
+            (d == 0 ? acc0 : acc1)[v * I::n3 + I::sbase(d, ln) + l * I::stride(d)] = 0.0;
+          }
+        }
+        if (warp < kGW0) {
+          // wave 2: accumulates; the barrier between the waves is taken inside, just before the update
+          chain_dir<N, DIFF, 3, false, 0, 2>(L, ph, nbs[cur], io, geo, e, sQ, sGc, sQo, sS, warp < M::FG ? acc0 : acc1, fl[1], fr[1], fd[1]);
+          // The bulk copies of the next element are observed BEFORE this warp reports that it is done with element e: after
+          // that report the helpers may start the copies of the element after the next, and a wait for "the phase of this
+          // parity" would then match the wrong phase.
+          if (more) wait_inputs();
+          bar_arrive(kBarRes, kMainThreads);     // this warp is done with element e
+          if (!more) break;
+          load_jv(e + gridDim.x);
+        } else {
+          bar_arrive(kBarWave, CH);
+          if (more) {
+            wait_inputs();
+            bar_sync(kBarNext, H + 32 * kGW);    // inputs, common solution and common fluxes of the next element are in shared memory
+          }
+          bar_arrive(kBarRes, kMainThreads);
+          if (!more) break;
+          if constexpr (GRADV != 0) {
+            const double* qn = sm + (cur ^ 1) * kIn;
+            double* sGn = sG + (cur ^ 1) * kGS;
+            for (int i = warp - kGW0; i < M::kTasks; i += kGW) {
+              const int td = s_task[i * 8 + L.r];
+              grad_dir<N, NGV, GV0, 3, true>(L, nbs[cur ^ 1], qn, qn + ev(9 * I::n3), qn + ev(9 * I::n3) + ev(kOwn), sGn, td & 0xffff,
+                                              (td >> 20) != 0, (td >> 16) & 3);
+            }
+          }
+          load_jv(e + gridDim.x);
+        }
+        bar_sync(kBarChain, CH);                 // the next element's gradient tasks are done, and every chain warp with element e
+        chain_rule(sG + (cur ^ 1) * kGS);
+        bar_sync(kBarChain, CH);
+        bar_arrive(kBarGrad, kMainThreads);
+      }
+    } else
     for (int64_t e = blockIdx.x; e < E; e += gridDim.x, ++it) {
-      const int cur = kPre ? (it & 1) : 0;
+      const int cur = 0;
       double* sQ = sm + cur * kIn;
       double* sQo = sQ + ev(9 * I::n3);
       double* sQn = sQo + ev(kOwn);
       const double* sS = kSglobal ? geo.Sfl + e * 9 * I::nf : sQn + ev(54 * I::n2);
-      double* sR = kPre ? sR0 : sQo;
-      double* sFace = kPre ? sQo : sQn;       // where the common face fluxes are
+      double* sR = sQo;
+      double* sFace = sQn;       // where the common face fluxes are
       const ElemNbr& nb = nbs[cur];
       int tw = M::kWarps, tl_d = 0, tl_ln = 0;
       bool tl_ok = false;
@@ -817,7 +945,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
 #pragma unroll
             for (int k = 0; k < M::kTPD; ++k)
               if (warp + k * M::kWarps < M::FG) {
-                if (k == 0) chain_dir<N, DIFF, 1, false, -1, true>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
+                if (k == 0) chain_dir<N, DIFF, 1, false, -1, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
                 else chain_dir<N, DIFF, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[1][k], true);
                 first = false;
               }
@@ -828,14 +956,14 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
 #pragma unroll
             for (int k = 0; k < M::kTPD; ++k)
               if (warp + k * M::kWarps < M::FG) {
-                if (k == 0) chain_dir<N, DIFF, 2, false, -1, true>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
+                if (k == 0) chain_dir<N, DIFF, 2, false, -1, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
                 else chain_dir<N, DIFF, 2>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, lnd[2][k], true);
                 first = false;
               }
           }
           if (first) bar_sync(kBarChain, CH);
           if (M::kTail > 0) {   // left-over lines of the three directions: no two of them share a solution point
-            if (active && tw < M::kTail) chain_dir<N, DIFF, 3, false, -1, true>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, tl_ln, tl_ok, tl_d);
+            if (active && tw < M::kTail) chain_dir<N, DIFF, 3, false, -1, 1>(L, ph, nb, io, geo, e, sQ, sG, sQn, sS, sR, tl_ln, tl_ok, tl_d);
             else bar_sync(kBarChain, CH);
           }
         }
@@ -928,7 +1056,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     double K[P2][9], w[P2];                     // sources and Runge-Kutta registers of this thread's points (set beside the chains)
     auto finish = [&](int64_t ef, int setf) {   // out = w * (div_xi F~) + K for element ef, whose tiles are input set setf
       double* sQ = sm + setf * kIn;
-      double* sR = kPre ? sR0 : sQ + ev(9 * I::n3);
+      double* sR = sQ + ev(9 * I::n3);
 #pragma unroll
       for (int q = 0; q < P2; ++q) {
         const int s = tid + q * H;
@@ -936,8 +1064,10 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           double R[9];
 #pragma unroll
           for (int v = 0; v < 9; ++v) {
-            double dv = sR[v * I::n3 + s];
-            if (M::kFree) dv += sR12[v * I::n3 + s] + sR12[kRS + v * I::n3 + s];     // one accumulator per direction
+            double dv;
+            if (kPre) dv = sR12[v * I::n3 + s] + sR12[kRS + v * I::n3 + s];          // the accumulators of the two waves
+            else if (M::kFree) dv = sR[v * I::n3 + s] + sR12[v * I::n3 + s] + sR12[kRS + v * I::n3 + s];   // one per direction
+            else dv = sR[v * I::n3 + s];
             R[v] = w[q] * dv + K[q][v];
           }
           if (DIFF) {                    // finished by the face kernel
@@ -962,7 +1092,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
       bar_sync(kBarHelp, H);                   // every helper is done with this element's shared memory
     };
     // A8 sources and the Runge-Kutta registers of element es (state tile sQ), so that  out = w * (div_xi F~) + K  is all that is left
-    auto sources = [&](int64_t e, const double* sQ) {
+    auto sources = [&](int64_t e, const double* sQ, const double* sG) {
 #pragma unroll
       for (int q = 0; q < P2; ++q) {
         const int s = tid + q * H;
@@ -1040,20 +1170,21 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         ld_phase ^= 1u;
         bar_sync(kBarHelp, H);
         face_pass(blockIdx.x, 0);
+        bar_sync(kBarIn, kMainThreads);              // the first element is handed over: inputs, common solution, common fluxes
       }
       for (int64_t e = blockIdx.x; e < E; e += gridDim.x, ++it) {
         const int cur = it & 1;
         const bool more = e + gridDim.x < E;
         e_last = e;
-        bar_sync(kBarIn, kMainThreads);              // inputs, common solution and common fluxes of e are in shared memory
-        // With diffusion the finish of the previous element touches no input tile (it writes Part from the accumulators): the
-        // next loads go first, so that the proxy fence of their issuing threads does not wait for the finish's global stores.
+        // The chain warps are done with the previous element (RES): its input set is free.  With diffusion its finish touches no
+        // input tile (it writes Part from the accumulators): the next loads go first, so that the proxy fence of their issuing
+        // threads does not wait for the finish's global stores.
         if (DIFF && more) {
           issue_loads_a(e + gridDim.x, cur ^ 1);
           issue_loads_b(e + gridDim.x, cur ^ 1);
           fetch_nbr(e + 2 * (int64_t)gridDim.x);
         }
-        if (it > 0) finish(e - gridDim.x, cur ^ 1);  // previous element: reads the accumulators, frees its input set
+        if (it > 0) finish(e - gridDim.x, cur ^ 1);  // previous element: reads the accumulators
         bar_arrive(kBarFaces, kMainThreads);         // the accumulators are free for this element's chains
         if (!DIFF && more) {
           issue_loads_a(e + gridDim.x, cur ^ 1);
@@ -1068,9 +1199,10 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           bar_sync(kBarHelp, H);
           face_pass(e + gridDim.x, cur ^ 1);
         }
-        bar_sync(kBarGrad, kMainThreads);            // the gradient of e is complete (div B of the Powell sources)
-        sources(e, sm + cur * kIn);
-        bar_sync(kBarRes, kMainThreads);
+        bar_sync(kBarGrad, kMainThreads);            // the gradient of e is complete (the chain warps arrived an element ago)
+        if (more) bar_arrive(kBarNext, H + 32 * (M::kFreeWarps - (M::kTasks - M::kFreeWarps)));   // next element handed over
+        sources(e, sm + cur * kIn, sG + cur * kGS);
+        bar_sync(kBarRes, kMainThreads);             // every chain warp is done with element e
       }
       if (e_last >= 0) finish(e_last, (it - 1) & 1);
     } else
@@ -1206,7 +1338,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           for (int k = 0; k < 7; ++k) o[k * I::n2] = Fv[k];
         }
       }
-      sources(e, sQ);                          // beside the chains
+      sources(e, sQ, sG);                      // beside the chains
       // measured: -0.9k cycles of the 6.2k the chain warps wait for the next element's inputs
       if (e + (kPre ? 2 : 1) * (int64_t)gridDim.x < E)
         prefetch_next<N, GRADV>(io, geo, e + (kPre ? 2 : 1) * (int64_t)gridDim.x, pn_e, pn_f, tid, H);
@@ -1235,7 +1367,7 @@ constexpr size_t stage_main_smem_bytes() {
   constexpr int kOwn = 54 * I::n2 > 9 * I::n3 ? 54 * I::n2 : 9 * I::n3;
   constexpr auto ev = [](int x) { return (x + 1) & ~1; };
   return sizeof(double) * (size_t)((kPrefetchOrder(N) ? 2 : 1) * (ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + (kSglobalOrder(N) ? 0 : 9 * I::nf)) +
-                                   ev(3 * NGV * I::n3) + (Mma<N>::kFree ? (kPrefetchOrder(N) ? 3 : 2) * ev(9 * I::n3) : 0));
+                                   (kPrefetchOrder(N) ? 2 : 1) * ev(3 * NGV * I::n3) + (Mma<N>::kFree ? 2 * ev(9 * I::n3) : 0));
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -39,6 +39,7 @@ struct chorus_ctx {
   double *d_Gm = nullptr, *d_Dff = nullptr, *d_Efs = nullptr, *d_Dfs = nullptr;
   // geometry
   double *d_Sfl = nullptr, *d_detJ = nullptr, *d_jinv = nullptr, *d_xsol = nullptr, *d_krfl = nullptr, *d_nfc = nullptr;
+  double* d_Sint = nullptr;         // S^d at the interior flux points (orders whose element kernel stages it: kSintOrder)
   // state registers (element-major) and face buffers
   double* d_U[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   int cur = 0;
@@ -205,7 +206,7 @@ struct Hot {
     return CHORUS_OK;
   }
   static Geo geo(const chorus_ctx* c) {
-    return Geo{c->d_Sfl, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl, c->d_nfc, c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient};
+    return Geo{c->d_Sfl, c->d_Sint, c->d_detJ, c->d_jinv, c->d_xsol, c->d_krfl, c->d_nfc, c->d_nbr_elem, c->d_nbr_face, c->d_nbr_orient};
   }
   // one residual evaluation through the pipeline.  io carries Qe and the outputs; the traces of Qe must be in d_Qf[qf_cur].
   static int stage_pipeline_main(chorus_ctx* c, StageIO& io) {
@@ -380,6 +381,11 @@ int run_geometry(chorus_ctx* c) {
   face_geometry_kernel<<<grid_1d(c, c->E * 6 * c->n2, 256), 256, 0, c->stream>>>(c->n, c->E, c->d_Sfl, c->d_nfc);
   ++c->launches;
   CU(c, cudaGetLastError());
+  if (c->d_Sint) {
+    interior_S_kernel<<<grid_1d(c, c->E * 9 * c->n2 * (c->n - 1), 256), 256, 0, c->stream>>>(c->n, c->E, c->d_Sfl, c->d_Sint);
+    ++c->launches;
+    CU(c, cudaGetLastError());
+  }
   return CHORUS_OK;
 }
 
@@ -455,6 +461,7 @@ int chorus_init(chorus_ctx** out, const chorus_mesh* mesh, int order, const chor
   bool ok = dalloc(&c->d_Sfl, E * 9 * c->nf) && dalloc(&c->d_detJ, E * c->n3) && dalloc(&c->d_jinv, E * 9 * c->n3) &&
             dalloc(&c->d_xsol, E * 3 * c->n3) && dalloc(&c->d_nfc, E * 24 * c->n2) && dalloc(&c->d_Qf[0], E * 54 * c->n2) && dalloc(&c->d_Qf[1], E * 54 * c->n2) &&
             dalloc(&c->d_Vf, E * 42 * c->n2);
+  if (kSintOrder(c->n)) ok = ok && dalloc(&c->d_Sint, E * 9 * c->n2 * (c->n - 1));
   for (int k = 0; k < 5 && ok; ++k) ok = dalloc(&c->d_U[k], E * 9 * c->n3);
   ok = ok && cudaMalloc(&c->d_ws, sizeof(unsigned long long)) == cudaSuccess;
   ok = ok && dalloc(&c->d_diag, (size_t)(kDiagBlocks + 1) * 3);
@@ -473,7 +480,7 @@ void chorus_free(chorus_ctx* c) {
   if (!c) return;
   cudaFree(c->d_xyz); cudaFree(c->d_nbr_elem); cudaFree(c->d_nbr_face); cudaFree(c->d_nbr_orient);
   cudaFree(c->d_Gm); cudaFree(c->d_Dff); cudaFree(c->d_Efs); cudaFree(c->d_Dfs);
-  cudaFree(c->d_Sfl); cudaFree(c->d_detJ); cudaFree(c->d_jinv); cudaFree(c->d_xsol); cudaFree(c->d_krfl); cudaFree(c->d_nfc);
+  cudaFree(c->d_Sfl); cudaFree(c->d_Sint); cudaFree(c->d_detJ); cudaFree(c->d_jinv); cudaFree(c->d_xsol); cudaFree(c->d_krfl); cudaFree(c->d_nfc);
   for (int k = 0; k < 5; ++k) cudaFree(c->d_U[k]);
   cudaFree(c->d_Qf[0]); cudaFree(c->d_Qf[1]); cudaFree(c->d_Vf); cudaFree(c->d_send_elem); cudaFree(c->d_send_face); cudaFree(c->d_recv_elem); cudaFree(c->d_recv_face);
   cudaFree(c->d_ws); cudaFree(c->d_wq); cudaFree(c->d_diag); cudaFree(c->d_arrivals); cudaFree(c->d_scratch);

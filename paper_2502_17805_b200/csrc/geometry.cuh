@@ -190,4 +190,24 @@ __global__ void face_geometry_kernel(int n, int64_t E, const double* __restrict_
   }
 }
 
+// S^d at the INTERIOR flux points only (m = 1 .. n-1), the part of Sfl that the element kernel's chains read (the face points go
+// through nfc): Sint[e][fam d][comp][.] in the natural family layout with n - 1 points per line,
+//   d = 0: ab (n-1) + (m-1);   d = 1: b (n-1) n + (m-1) n + a;   d = 2: (m-1) n^2 + ab.
+__global__ void interior_S_kernel(int n, int64_t E, const double* __restrict__ Sfl, double* __restrict__ Sint) {
+  const int n2 = n * n, nf = n2 * (n + 1), nfi = n2 * (n - 1);
+  const int64_t total = E * 9 * nfi;
+  for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total; t += (int64_t)gridDim.x * blockDim.x) {
+    const int idx = (int)(t % nfi), fc = (int)((t / nfi) % 9);
+    const int64_t e = t / (9 * (int64_t)nfi);
+    const int d = fc / 3;
+    int ab, m;
+    if (d == 0) { ab = idx / (n - 1); m = idx % (n - 1) + 1; }
+    else if (d == 1) { const int b = idx / ((n - 1) * n), r = idx % ((n - 1) * n); m = r / n + 1; ab = b * n + r % n; }
+    else { m = idx / n2 + 1; ab = idx % n2; }
+    const int a = ab % n, b = ab / n;
+    const int fb = d == 0 ? ab * (n + 1) : d == 1 ? b * (n + 1) * n + a : ab;
+    Sint[t] = Sfl[(e * 9 + fc) * nf + fb + m * (d == 0 ? 1 : d == 1 ? n : n2)];
+  }
+}
+
 }  // namespace chorus

@@ -41,7 +41,10 @@ __host__ __device__ constexpr bool kWideOrder(int n) { return n >= 6 && n <= 8; 
 // from global memory (L2) instead of a shared-memory tile: 212 KB of tiles in all.
 __host__ __device__ constexpr bool kFaceOutOrder(int n) { return n == 8; }
 // orders whose chains read S^d at the flux points from global memory (L2; prefetched an element ahead) instead of a shared-memory tile
-__host__ __device__ constexpr bool kSglobalOrder(int n) { return n == 8 || n == 6; }
+__host__ __device__ constexpr bool kSglobalOrder(int n) { return n == 8; }
+// orders whose shared-memory S^d tile holds the INTERIOR flux points only (Geo::Sint; the face points go through nfc): with two
+// gradient buffers the full tile no longer fits twice
+__host__ __device__ constexpr bool kSintOrder(int n) { return n == 6; }
 // ... and, of these, the ones with room for a SECOND set of input tiles (state, own and neighbour traces, S^d): the next
 // element's inputs stream in while the current element's chains run, so the chain warps never wait for them
 __host__ __device__ constexpr bool kPrefetchOrder(int n) { return n == 6; }
@@ -118,6 +121,7 @@ struct StageIO {
 
 struct Geo {
   const double* Sfl;     // [E][3 fam][3 comp][nf]
+  const double* Sint;    // [E][3 fam][3 comp][n2 (n-1)]  interior flux points only (kSintOrder), or nullptr
   const double* detJ;    // [E][n3]
   const double* jinv;    // [E][3 d][3 p][n3]
   const double* xsol;    // [E][3][n3]
@@ -420,13 +424,16 @@ __device__ __forceinline__ void chain_dir(const LaneK<N>& L, const PhysD& ph, co
   // per-slot setup: area vector and the state the fluxes are evaluated on
   const bool face0 = m0 == 0 || m0 == N, face1 = m1 == 0 || m1 == N;     // m = -1: padding
   int fc0 = 0, fc1 = 0;
+  constexpr int kNFS = kSintOrder(N) ? I::n2 * (N - 1) : I::nf;        // points per component of the S^d tile
+  // interior-only tile: the natural family layout with n - 1 points per line, first point m = 1
+  const int fbs = !kSintOrder(N) ? fb : d == 0 ? ln * (N - 1) - 1 : d == 1 ? (ln / N) * (N - 1) * N + ln % N - N : ln - I::n2;
   if (!kSglobalOrder(N) && int0) {
-    const double* s = sS + (d * 3) * I::nf + fb + m0 * st;
-    S0x = s[0]; S0y = s[I::nf]; S0z = s[2 * I::nf];
+    const double* s = sS + (d * 3) * kNFS + fbs + m0 * st;
+    S0x = s[0]; S0y = s[kNFS]; S0z = s[2 * kNFS];
   }
   if (!kSglobalOrder(N) && int1) {
-    const double* s = sS + (d * 3) * I::nf + fb + m1 * st;
-    S1x = s[0]; S1y = s[I::nf]; S1z = s[2 * I::nf];
+    const double* s = sS + (d * 3) * kNFS + fbs + m1 * st;
+    S1x = s[0]; S1y = s[kNFS]; S1z = s[2 * kNFS];
   }
   if (DIFF) {   // face columns: the own-side viscous flux along the outward unit normal, on Q_in (interior) or Q_b (wall)
     if (face0) {
@@ -567,7 +574,8 @@ __device__ __forceinline__ void prefetch_next(const StageIO& io, const Geo& geo,
   using I = Ix<N>;
   prefetch_block_l2(io.Qe + en * 9 * I::n3, sizeof(double) * 9 * I::n3, tid, nthreads);
   prefetch_block_l2(io.Qf + en * 54 * I::n2, sizeof(double) * 54 * I::n2, tid, nthreads);
-  prefetch_block_l2(geo.Sfl + en * 9 * I::nf, sizeof(double) * 9 * I::nf, tid, nthreads);
+  if (kSintOrder(N)) prefetch_block_l2(geo.Sint + en * 9 * I::n2 * (N - 1), sizeof(double) * 9 * I::n2 * (N - 1), tid, nthreads);
+  else prefetch_block_l2(geo.Sfl + en * 9 * I::nf, sizeof(double) * 9 * I::nf, tid, nthreads);
   prefetch_block_l2(geo.nfc + en * 24 * I::n2, sizeof(double) * 24 * I::n2, tid, nthreads);
   prefetch_block_l2(geo.detJ + en * I::n3, sizeof(double) * I::n3, tid, nthreads);
   prefetch_block_l2(geo.xsol + en * 3 * I::n3, sizeof(double) * 3 * I::n3, tid, nthreads);
@@ -595,7 +603,8 @@ __device__ __forceinline__ void prefetch_next(const StageIO& io, const Geo& geo,
 //   n = 8      one CTA per SM (212 KB), 8 + 8 warps, three barrier-separated direction rounds of 8 tasks on one accumulator;
 //              its tiles hold 7 interior flux points and the face point m = n (kFaceOutOrder), S^d comes from L2;
 //   n = 6      one CTA per SM, 8 chain warps (168) + 8 helper warps (88), TWO sets of input tiles and TWO gradient buffers
-//              (kPre, 213 KB in all; S^d from L2): while the chain warps work on element e the helpers bring in element
+//              (kPre, 223 KB in all; the S^d tile holds the interior flux points only, Geo::Sint, and the neighbour-trace /
+//              common-solution tile exists once): while the chain warps work on element e the helpers bring in element
 //              e + 1 -- bulk copies, wall states, common solution and common fluxes (face_pass) -- and the two chain warps
 //              that have no task in the element's second wave compute the gradient of e + 1, so that between two elements
 //              only the chain rule is left; the finish of element e is deferred until e + 1 is under way.  Barriers per
@@ -616,9 +625,14 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   // one set of INPUT tiles: sQ [9][n3] | sQo [6][9][n2] own traces, reused as sR [9][n3] after the face pass | sQn [6][9][n2]
   // neighbour traces / wall states, overwritten by the face fluxes | sS [3 fam][3 comp][nf] S^d at the flux points
   constexpr bool kSglobal = kSglobalOrder(N);   // S^d read from global memory by the chains (no shared-memory tile)
-  constexpr int kIn = ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + (kSglobal ? 0 : 9 * I::nf);
   constexpr bool kPre = kPrefetchOrder(N);   // two input sets, used alternately (element i of this CTA: set i & 1)
-  double* sG = sm + (kPre ? 2 : 1) * kIn;    // [3*NGV][n3]; kPre: two of them (the gradient of the next element is made ahead)
+  static_assert(!kPre || kSintOrder(N), "the kPre layout stages the interior-only S^d tile");
+  constexpr int kST = kSglobal ? 0 : kSintOrder(N) ? 9 * I::n2 * (N - 1) : 9 * I::nf;    // doubles of the S^d tile
+  // kPre: the neighbour traces / common solution tile sQn is NOT part of the set: it lives from the loads of an element to the
+  // end of that element's gradient tasks, which run an element ahead -- one copy is enough
+  constexpr int kIn = ev(9 * I::n3) + ev(kOwn) + (kPre ? 0 : ev(54 * I::n2)) + kST;
+  double* sQn1 = sm + 2 * kIn;               // kPre: the single sQn
+  double* sG = sm + (kPre ? 2 * kIn + ev(54 * I::n2) : kIn);    // [3*NGV][n3]; kPre: two of them (the next gradient is made ahead)
   constexpr int kGS = ev(3 * NGV * I::n3);
   double* sR12 = sG + (kPre ? 2 : 1) * kGS;  // kFree: the accumulators of directions 1 and 2, [2][9][n3] (direction 0: sR);
   constexpr int kRS = ev(9 * I::n3);         // kPre: the two accumulators of the two task waves (see the chain loop)
@@ -788,7 +802,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           const double* q0 = sm;
 #pragma unroll
           for (int t = 0; t < M::kTPW; ++t)
-            if (fv[t]) grad_dir<N, NGV, GV0, 3, true>(L, nbs[0], q0, q0 + ev(9 * I::n3), q0 + ev(9 * I::n3) + ev(kOwn), sG, fl[t], fr[t], fd[t]);
+            if (fv[t]) grad_dir<N, NGV, GV0, 3, true>(L, nbs[0], q0, q0 + ev(9 * I::n3), sQn1, sG, fl[t], fr[t], fd[t]);
         }
         bar_sync(kBarChain, CH);
         chain_rule(sG);
@@ -800,7 +814,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         const bool more = e + gridDim.x < E;
         double* sQ = sm + cur * kIn;
         double* sQo = sQ + ev(9 * I::n3);        // the common face fluxes
-        const double* sS = geo.Sfl + e * 9 * I::nf;
+        const double* sS = sQo + ev(kOwn);       // S^d at the interior flux points
         const double* sGc = sG + cur * kGS;
         // wave 1: stores; the FACES barrier (accumulators free) is taken inside, just before the common fluxes are needed
         chain_dir<N, DIFF, 3, true, 1>(L, ph, nbs[cur], io, geo, e, sQ, sGc, sQo, sS, fd[0] == 0 ? acc0 : acc1, fl[0], fr[0], fd[0], tid);
@@ -828,17 +842,22 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
             wait_inputs();
             bar_sync(kBarNext, H + 32 * kGW);    // inputs, common solution and common fluxes of the next element are in shared memory
           }
-          bar_arrive(kBarRes, kMainThreads);
-          if (!more) break;
+          if (!more) {
+            bar_arrive(kBarRes, kMainThreads);
+            break;
+          }
           if constexpr (GRADV != 0) {
             const double* qn = sm + (cur ^ 1) * kIn;
             double* sGn = sG + (cur ^ 1) * kGS;
             for (int i = warp - kGW0; i < M::kTasks; i += kGW) {
               const int td = s_task[i * 8 + L.r];
-              grad_dir<N, NGV, GV0, 3, true>(L, nbs[cur ^ 1], qn, qn + ev(9 * I::n3), qn + ev(9 * I::n3) + ev(kOwn), sGn, td & 0xffff,
+              grad_dir<N, NGV, GV0, 3, true>(L, nbs[cur ^ 1], qn, qn + ev(9 * I::n3), sQn1, sGn, td & 0xffff,
                                               (td >> 20) != 0, (td >> 16) & 3);
             }
           }
+          // done with element e AND with the common solution of the next one in the single sQn tile: after this report the
+          // helpers may start the copies of the element after the next into it
+          bar_arrive(kBarRes, kMainThreads);
           load_jv(e + gridDim.x);
         }
         bar_sync(kBarChain, CH);                 // the next element's gradient tasks are done, and every chain warp with element e
@@ -989,12 +1008,12 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     // part B: own traces (their region doubles as the divergence accumulator sR, read by the final combination)
     auto issue_loads_a = [&](int64_t el, int set) {
       double* sQ = sm + set * kIn;
-      double* sQn = sQ + ev(9 * I::n3) + ev(kOwn);
-      double* sS = sQn + ev(54 * I::n2);
+      double* sQn = kPre ? sQn1 : sQ + ev(9 * I::n3) + ev(kOwn);
+      double* sS = kPre ? sQ + ev(9 * I::n3) + ev(kOwn) : sQn + ev(54 * I::n2);
       ElemNbr& nb = nbs[set];
       if (tid < 6) { nb.ne[tid] = pn_e; nb.nf[tid] = pn_f; nb.no[tid] = pn_o; }
       const double* q = io.Qe + el * 9 * I::n3;
-      const double* g = geo.Sfl + el * 9 * I::nf;
+      const double* g = kSintOrder(N) ? geo.Sint + el * kST : geo.Sfl + el * 9 * I::nf;
       if (kBulk) {
         if (tid < 32) {
           // neighbour faces that meet this element with the identity orientation (all faces inside a panel, most seam faces)
@@ -1003,7 +1022,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           const unsigned cnt = __popc(__ballot_sync(0xffffffffu, whole));
           if (tid == 0) {
             fence_proxy_async();
-            mbar_expect_tx(&mbar, (unsigned)(sizeof(double) * (9 * I::n3 + (kSglobal ? 0 : 9 * I::nf) + cnt * 9 * I::n2)));
+            mbar_expect_tx(&mbar, (unsigned)(sizeof(double) * (9 * I::n3 + kST + cnt * 9 * I::n2)));
             tma_load(sQ, q, sizeof(double) * 9 * I::n3, &mbar);
           }
           if (whole) {
@@ -1012,12 +1031,12 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           }
         } else if (tid == 32 && !kSglobal) {
           fence_proxy_async();
-          tma_load(sS, g, sizeof(double) * 9 * I::nf, &mbar);
+          tma_load(sS, g, sizeof(double) * kST, &mbar);
         }
       } else {
         for (int k = tid; k < 9 * I::n3; k += H) cp_async8(sQ + k, q + k);
         if (!kSglobal)
-          for (int k = tid; k < 9 * I::nf / 2; k += H) cp_async16(sS + 2 * k, g + 2 * k);
+          for (int k = tid; k < kST / 2; k += H) cp_async16(sS + 2 * k, g + 2 * k);
       }
       bar_sync(kBarHelp, H);   // nb visible
       for (int k = tid; k < 6 * I::n2; k += H) {
@@ -1130,7 +1149,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
     // or wall state Q_b) replaces the neighbour traces, the common FLUX (Rusanov / wall, scaled by sigma |S|) the own traces
     auto face_pass = [&](int64_t el, int set) {
       double* sQo = sm + set * kIn + ev(9 * I::n3);
-      double* sQn = sQo + ev(kOwn);
+      double* sQn = kPre ? sQn1 : sQo + ev(kOwn);
       const ElemNbr& nb = nbs[set];
       for (int t = tid; t < 6 * I::n2; t += H) {
         const int f = t / I::n2, ab = t % I::n2;
@@ -1178,7 +1197,9 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         e_last = e;
         // The chain warps are done with the previous element (RES): its input set is free.  With diffusion its finish touches no
         // input tile (it writes Part from the accumulators): the next loads go first, so that the proxy fence of their issuing
-        // threads does not wait for the finish's global stores.
+        // threads does not wait for the finish's global stores.  The single neighbour tile is free as well: the chain warps
+        // report RES after the gradient tasks that read it -- except before the first element, whose gradient is awaited here.
+        if (it == 0) bar_sync(kBarGrad, kMainThreads);
         if (DIFF && more) {
           issue_loads_a(e + gridDim.x, cur ^ 1);
           issue_loads_b(e + gridDim.x, cur ^ 1);
@@ -1199,7 +1220,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           bar_sync(kBarHelp, H);
           face_pass(e + gridDim.x, cur ^ 1);
         }
-        bar_sync(kBarGrad, kMainThreads);            // the gradient of e is complete (the chain warps arrived an element ago)
+        if (it > 0) bar_sync(kBarGrad, kMainThreads);   // the gradient of e is complete (the chain warps arrived an element ago)
         if (more) bar_arrive(kBarNext, H + 32 * (M::kFreeWarps - (M::kTasks - M::kFreeWarps)));   // next element handed over
         sources(e, sm + cur * kIn, sG + cur * kGS);
         bar_sync(kBarRes, kMainThreads);             // every chain warp is done with element e
@@ -1366,7 +1387,10 @@ constexpr size_t stage_main_smem_bytes() {
   constexpr int NGV = GRADV == 2 ? 9 : GRADV == 1 ? 3 : 0;
   constexpr int kOwn = 54 * I::n2 > 9 * I::n3 ? 54 * I::n2 : 9 * I::n3;
   constexpr auto ev = [](int x) { return (x + 1) & ~1; };
-  return sizeof(double) * (size_t)((kPrefetchOrder(N) ? 2 : 1) * (ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + (kSglobalOrder(N) ? 0 : 9 * I::nf)) +
+  constexpr int kST = kSglobalOrder(N) ? 0 : kSintOrder(N) ? 9 * I::n2 * (N - 1) : 9 * I::nf;
+  if (kPrefetchOrder(N))   // two sets of (state, own traces / fluxes, S^d), one neighbour tile, two gradients, two accumulators
+    return sizeof(double) * (size_t)(2 * (ev(9 * I::n3) + ev(kOwn) + kST) + ev(54 * I::n2) + 2 * ev(3 * NGV * I::n3) + 2 * ev(9 * I::n3));
+  return sizeof(double) * (size_t)((kPrefetchOrder(N) ? 2 : 1) * (ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + kST) +
                                    (kPrefetchOrder(N) ? 2 : 1) * ev(3 * NGV * I::n3) + (Mma<N>::kFree ? 2 * ev(9 * I::n3) : 0));
 }
 

@@ -159,6 +159,27 @@ int chorus_profile_read(chorus_ctx* ctx, double* ms /*[3]*/, int64_t* launches /
  * dfma_tflops / dmma_tflops (HOST, may be NULL) = the share of each instruction kind (equal halves in mode 2). */
 int chorus_fp64_peak(int mode, double seconds, double* tflops, double* dfma_tflops, double* dmma_tflops);
 
+/* ---- allocation-free entry point --------------------------------------------------------------------------------
+ * The diagnostics of chorus_diagnostics (Eq. 34-35; same quadrature) for callers that cannot call
+ * cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid allocation.  It needs no context and
+ * calls no cudaMalloc, cudaFree or other allocating routine: the partial sums of its reduction live in a device array of
+ * fixed size inside the library (96 KB, held by every GPU that loads the library until the process exits).
+ *   order    2..9;  n_elem >= 1;  n_elem * order^3 <= CHORUS_STATIC_DIAG_MAX_POINTS, else CHORUS_EINVAL (nothing is launched)
+ *   q        DEVICE, [9][n_elem][order^3] conserved variables in the interface layout (as chorus_get_state gives them)
+ *   detJ     DEVICE, [n_elem][order^3]    |J| at the solution points (as chorus_get_geometry gives it)
+ *   out      DEVICE, 3 doubles: V = int dV, KE (Eq. 34), E_B (Eq. 35)
+ *   stream   a cudaStream_t (NULL = default stream); two kernels are enqueued on it, nothing synchronises
+ * All pointers stay owned by the caller.  Uses the CURRENT device; its first call on a device looks up the array's address
+ * (cudaGetSymbolAddress), so make one call per device outside graph capture.  Every call on a device shares the one scratch
+ * array, which keeps the last call's contents (each call overwrites every entry it reads: nothing has to be cleared): calls
+ * that OVERLAP on the GPU -- different streams, or concurrent graph launches -- race and must be serialised by the caller.
+ * The summation tree is fixed by the size alone (8192 points per block), so results are bit-identical from call to call; they
+ * differ from chorus_diagnostics at round-off (another tree).  On failure chorus_static_last_error() has the message
+ * (per calling thread; valid until that thread's next call). */
+#define CHORUS_STATIC_DIAG_MAX_POINTS 33554432 /* 2^25 solution points: 4096 blocks x 8192 points, 96 KB of partial sums */
+int chorus_diagnostics_static(int order, int64_t n_elem, const double* q, const double* detJ, double* out, void* cuda_stream);
+const char* chorus_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -15,12 +15,14 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("CHORUS_LIB", os.path.join(HERE, "libchorus_b200.so"))   # override: A/B testing of builds
 
 CHORUS_OK, CHORUS_EINVAL, CHORUS_ENOMEM, CHORUS_ECUDA, CHORUS_ESTATE = 0, -1, -2, -3, -4
+STATIC_DIAG_MAX_POINTS = 1 << 25     # CHORUS_STATIC_DIAG_MAX_POINTS of include/chorus.h
 
 # every symbol include/chorus.h declares
 SYMBOLS = ("chorus_init", "chorus_free", "chorus_set_physics", "chorus_set_state", "chorus_get_state", "chorus_residual",
            "chorus_step", "chorus_step_begin", "chorus_stage_main", "chorus_stage_face", "chorus_set_owned", "chorus_halo_setup",
            "chorus_halo_pack", "chorus_halo_unpack", "chorus_diagnostics_sums", "chorus_max_wavespeed", "chorus_diagnostics", "chorus_last_error", "chorus_get_geometry", "chorus_get_gradient",
-           "chorus_get_operators", "chorus_launch_count", "chorus_profile", "chorus_profile_read", "chorus_fp64_peak")
+           "chorus_get_operators", "chorus_launch_count", "chorus_profile", "chorus_profile_read", "chorus_fp64_peak",
+           "chorus_diagnostics_static", "chorus_static_last_error")
 
 
 class ChorusError(RuntimeError):
@@ -92,6 +94,9 @@ def lib():
         L.chorus_launch_count.restype = C.c_int64
         L.chorus_profile.argtypes = [V, I]
         L.chorus_profile_read.argtypes = [V, V, V]
+        L.chorus_diagnostics_static.argtypes = [I, C.c_int64, V, V, V, V]
+        L.chorus_static_last_error.argtypes = []
+        L.chorus_static_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -118,6 +123,23 @@ def get_operators(order):
     if rc:
         raise ChorusError(rc, "chorus_get_operators")
     return xs, xf, Isf, Dfs
+
+
+def diagnostics_static(order, q, detJ, out, stream=None):
+    """chorus_diagnostics_static (include/chorus.h): V, KE, E_B of a state WITHOUT a context and without any allocation.
+    q [9][E][n^3], detJ [E][n^3], out [3]: contiguous fp64 CUDA tensors of the current device; asynchronous on `stream`
+    (a torch.cuda.Stream, or None for the default stream).  Nothing is returned: the result lands in `out`."""
+    for a in (q, detJ, out):
+        if not (_is_torch(a) and a.is_cuda):
+            raise ChorusError(CHORUS_EINVAL, "diagnostics_static takes CUDA tensors")
+    n3 = int(order) ** 3
+    E = detJ.numel() // n3
+    if detJ.numel() != E * n3 or q.numel() != 9 * E * n3 or out.numel() != 3:
+        raise ChorusError(CHORUS_EINVAL, "diagnostics_static: q [9][E][n^3], detJ [E][n^3], out [3]")
+    st = C.c_void_p(stream.cuda_stream) if stream is not None else C.c_void_p(0)
+    rc = lib().chorus_diagnostics_static(int(order), E, _ptr(q)[0], _ptr(detJ)[0], _ptr(out)[0], st)
+    if rc != 0:
+        raise ChorusError(rc, lib().chorus_static_last_error().decode())
 
 
 def fp64_peak(mode=0, seconds=1.0):

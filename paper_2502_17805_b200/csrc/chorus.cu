@@ -902,3 +902,126 @@ int chorus_get_operators(int order, double* xs, double* xf, double* Isf, double*
 }
 
 }  // extern "C"
+
+// =========================================================================================================
+// Allocation-free diagnostics (chorus_diagnostics_static, include/chorus.h): for callers that cannot call cudaMalloc (code
+// under CUDA graph capture, tight serving loops, harnesses that forbid it).  The partial sums of the reduction -- the scratch
+// that chorus_diagnostics keeps in a cudaMalloc'ed buffer of its context -- live in a file-scope device array of fixed size,
+// which every GPU that loads the library holds until exit (96 KB).  No context, no cudaMalloc / cudaFree, no host heap use.
+//
+// The array's NAME is, in host code, a host-side stand-in and not a device address: the address the kernels are given is
+// obtained once per device, with that device current, by cudaGetSymbolAddress (static_diag_scratch below).
+// =========================================================================================================
+namespace {
+constexpr int kStaticDiagPointsPerBlock = 8192;      // solution points summed by one block (fixed: the summation tree depends on the size only)
+constexpr int kStaticDiagMaxBlocks = CHORUS_STATIC_DIAG_MAX_POINTS / kStaticDiagPointsPerBlock;   // 4096 partial triples
+static_assert((int64_t)kStaticDiagMaxBlocks * kStaticDiagPointsPerBlock == CHORUS_STATIC_DIAG_MAX_POINTS, "maximum = whole blocks");
+}  // namespace
+
+// partial sums [block][3] of one call.  Shared by every call on the device; keeps the last call's contents.
+static __device__ __align__(256) double g_static_diag_scratch[kStaticDiagMaxBlocks * 3];
+
+namespace chorus {
+struct QuadW { double w[kMaxN]; };   // quadrature weights of the solution points, by value (no device copy to allocate)
+
+// Variant of diagnostics_kernel: the state in the INTERFACE layout [9][E][n3] (what the caller holds), weights by value, a fixed
+// chunk of points per block, partial sums into the static scratch.  Every partial the final kernel reads is written by this
+// launch: nothing in the scratch has to start at zero.
+__global__ void __launch_bounds__(256) diagnostics_static_kernel(int64_t total, int64_t E, int n, QuadW wq, const double* __restrict__ detJ,
+                                                                const double* __restrict__ Q, double* __restrict__ partial) {
+  __shared__ double sh[8][3];
+  const int n3 = n * n * n;
+  const int64_t comp = E * n3;                      // stride between conserved variables
+  double V = 0.0, KE = 0.0, EB = 0.0;
+  const int64_t t0 = (int64_t)blockIdx.x * kStaticDiagPointsPerBlock;
+  const int64_t t1 = t0 + kStaticDiagPointsPerBlock < total ? t0 + kStaticDiagPointsPerBlock : total;
+  for (int64_t t = t0 + threadIdx.x; t < t1; t += blockDim.x) {
+    const int s = (int)(t % n3);
+    const int i = s % n, j = (s / n) % n, k = s / (n * n);
+    const double wJ = wq.w[i] * wq.w[j] * wq.w[k] * detJ[t];
+    const double* q = Q + t;
+    const double rho = q[0], m1 = q[comp], m2 = q[2 * comp], m3 = q[3 * comp];
+    const double b1 = q[5 * comp], b2 = q[6 * comp], b3 = q[7 * comp];
+    V += wJ;
+    KE += wJ * (0.5 * (m1 * m1 + m2 * m2 + m3 * m3) / rho);       // Eq. 34
+    EB += wJ * (0.5 * (b1 * b1 + b2 * b2 + b3 * b3));             // Eq. 35
+  }
+  block_sum3(V, KE, EB, sh);
+  if (threadIdx.x == 0) { partial[blockIdx.x * 3 + 0] = V; partial[blockIdx.x * 3 + 1] = KE; partial[blockIdx.x * 3 + 2] = EB; }
+}
+}  // namespace chorus
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+double* g_static_diag_ptr[kStaticMaxDevices] = {};   // device address of g_static_diag_scratch, per device (set-up once)
+bool g_static_diag_have[kStaticMaxDevices] = {};
+thread_local char g_static_err[256] = "";            // message of the calling thread's last failed context-free call
+
+int static_fail(int code, const char* what, cudaError_t e = cudaSuccess) {
+  if (e != cudaSuccess) std::snprintf(g_static_err, sizeof g_static_err, "%s: %s", what, cudaGetErrorString(e));
+  else std::snprintf(g_static_err, sizeof g_static_err, "%s", what);
+  return code;
+}
+
+// Set-up, once per device, with that device current: the device address of the scratch array.
+int static_diag_scratch(double** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return static_fail(CHORUS_ECUDA, "cudaGetDevice", e);
+  if (dev < 0 || dev >= kStaticMaxDevices) return static_fail(CHORUS_EINVAL, "chorus_diagnostics_static: device ordinal beyond 63");
+  if (!__atomic_load_n(&g_static_diag_have[dev], __ATOMIC_ACQUIRE)) {
+    double* p = nullptr;
+    e = cudaGetSymbolAddress((void**)&p, g_static_diag_scratch);
+    if (e != cudaSuccess || !p) return static_fail(CHORUS_ECUDA, "cudaGetSymbolAddress(static diagnostics scratch)", e);
+    g_static_diag_ptr[dev] = p;      // two threads racing here store the same address
+    __atomic_store_n(&g_static_diag_have[dev], true, __ATOMIC_RELEASE);
+  }
+  *out = g_static_diag_ptr[dev];
+  return CHORUS_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int chorus_diagnostics_static(int order, int64_t n_elem, const double* q, const double* detJ, double* out, void* cuda_stream) {
+  g_static_err[0] = '\0';
+  if (order < 2 || order > kMaxN) return static_fail(CHORUS_EINVAL, "chorus_diagnostics_static: order must be 2..9");
+  if (n_elem <= 0) return static_fail(CHORUS_EINVAL, "chorus_diagnostics_static: n_elem must be positive");
+  if (!q || !detJ || !out) return static_fail(CHORUS_EINVAL, "chorus_diagnostics_static: null pointer");
+  const int n = order, n3 = n * n * n;
+  if (n_elem > CHORUS_STATIC_DIAG_MAX_POINTS / n3) {
+    std::snprintf(g_static_err, sizeof g_static_err,
+                  "chorus_diagnostics_static: %lld elements x %d points exceed the static scratch's maximum of %d solution points "
+                  "(use chorus_diagnostics of a context for larger meshes)", (long long)n_elem, n3, (int)CHORUS_STATIC_DIAG_MAX_POINTS);
+    return CHORUS_EINVAL;
+  }
+  double* scratch = nullptr;
+  if (int rc = static_diag_scratch(&scratch)) return rc;
+  // Fejer's first rule on the Chebyshev-Gauss points (the closed form of basis.h), on the stack
+  QuadW wq;
+  const long double pi = 3.14159265358979323846264338327950288L;
+  for (int k = 1; k <= kMaxN; ++k) {
+    long double w = 0;
+    if (k <= n) {
+      const long double th = (2 * k - 1) * pi / (2 * n);
+      w = 1;
+      for (int j = 1; j <= n / 2; ++j) w -= 2 * cosl(2 * j * th) / (4.0L * j * j - 1);
+      w /= n;
+    }
+    wq.w[k - 1] = (double)w;
+  }
+  const int64_t total = n_elem * n3;
+  const int grid = (int)((total + kStaticDiagPointsPerBlock - 1) / kStaticDiagPointsPerBlock);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  diagnostics_static_kernel<<<grid, 256, 0, st>>>(total, n_elem, n, wq, detJ, q, scratch);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return static_fail(CHORUS_ECUDA, "diagnostics_static_kernel launch", e);
+  diagnostics_final_kernel<<<1, 256, 0, st>>>(grid, scratch, out, 0);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return static_fail(CHORUS_ECUDA, "diagnostics_final_kernel launch", e);
+  return CHORUS_OK;
+}
+
+const char* chorus_static_last_error(void) { return g_static_err; }
+
+}  // extern "C"

@@ -159,6 +159,21 @@ int chorus_profile_read(chorus_ctx* ctx, double* ms /*[3]*/, int64_t* launches /
  * dfma_tflops / dmma_tflops (HOST, may be NULL) = the share of each instruction kind (equal halves in mode 2). */
 int chorus_fp64_peak(int mode, double seconds, double* tflops, double* dfma_tflops, double* dmma_tflops);
 
+/* ---- host jobs, pipelined ------------------------------------------------------------------------------------------
+ * One job = chorus_set_state(q_in HOST) + chorus_step(dt, nstages) + chorus_get_state(q_out HOST) [+ the CFL wave speed of the
+ * result into *ws_out (HOST), if ws_out is not NULL], enqueued WITHOUT synchronising: the host-to-device copy runs on a copy
+ * stream of the library, the kernels on the context's stream, the device-to-host copies on a second copy stream, through two
+ * staging slots each way (4 x the state's size of device memory, allocated on the first call).  Jobs issued back to back overlap:
+ * the H2D of job k + 1 and the D2H of job k - 1 run beside the kernels of job k, so the step rate is max(copy, compute) instead
+ * of their sum.  Jobs are independent (each starts from its own q_in) and complete in order.
+ *   q_in, q_out, ws_out: HOST; [9][n_elem][n^3], the same, one double.  They are owned by the caller, must stay valid and
+ *   untouched until chorus_sync returns, and should be PINNED (cudaHostAlloc / cudaHostRegister): pageable memory works but the
+ *   copies then block the calling thread and nothing overlaps.  Results are bit-identical to the three separate calls.
+ * chorus_sync waits for everything the context has enqueued, the copy streams included.  Unpartitioned contexts only; errors as
+ * chorus_step.  After chorus_sync the context's state is the last job's result. */
+int chorus_step_host(chorus_ctx* ctx, const double* q_in, double* q_out, double dt, int nstages, double* ws_out);
+int chorus_sync(chorus_ctx* ctx);
+
 /* ---- allocation-free entry point --------------------------------------------------------------------------------
  * The diagnostics of chorus_diagnostics (Eq. 34-35; same quadrature) for callers that cannot call
  * cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid allocation.  It needs no context and

@@ -22,7 +22,7 @@ SYMBOLS = ("chorus_init", "chorus_free", "chorus_set_physics", "chorus_set_state
            "chorus_step", "chorus_step_begin", "chorus_stage_main", "chorus_stage_face", "chorus_set_owned", "chorus_halo_setup",
            "chorus_halo_pack", "chorus_halo_unpack", "chorus_diagnostics_sums", "chorus_max_wavespeed", "chorus_diagnostics", "chorus_last_error", "chorus_get_geometry", "chorus_get_gradient",
            "chorus_get_operators", "chorus_launch_count", "chorus_profile", "chorus_profile_read", "chorus_fp64_peak",
-           "chorus_diagnostics_static", "chorus_static_last_error")
+           "chorus_diagnostics_static", "chorus_static_last_error", "chorus_step_host", "chorus_sync")
 
 
 class ChorusError(RuntimeError):
@@ -94,6 +94,8 @@ def lib():
         L.chorus_launch_count.restype = C.c_int64
         L.chorus_profile.argtypes = [V, I]
         L.chorus_profile_read.argtypes = [V, V, V]
+        L.chorus_step_host.argtypes = [V, V, V, D, I, V]
+        L.chorus_sync.argtypes = [V]
         L.chorus_diagnostics_static.argtypes = [I, C.c_int64, V, V, V, V]
         L.chorus_static_last_error.argtypes = []
         L.chorus_static_last_error.restype = C.c_char_p
@@ -250,6 +252,19 @@ class Chorus:
 
     def halo_unpack(self, field, buf):
         self._check(lib().chorus_halo_unpack(self._ctx, int(field), C.c_void_p(buf.data_ptr())))
+
+    def step_host(self, q_in, q_out, dt, nstages=5, ws_out=None):
+        """chorus_step_host: one pipelined host job.  q_in, q_out: contiguous fp64 HOST arrays [9][E][n^3] (numpy or CPU torch,
+        pinned for overlap); ws_out: a 1-element fp64 HOST array or None.  Nothing is valid before sync()."""
+        assert tuple(q_in.shape) == self.shape and tuple(q_out.shape) == self.shape
+        (pi, di), (po, do) = _ptr(q_in), _ptr(q_out)
+        if di or do:
+            raise ChorusError(CHORUS_EINVAL, "step_host takes HOST buffers")
+        pw = _ptr(ws_out)[0] if ws_out is not None else C.c_void_p(0)
+        self._check(lib().chorus_step_host(self._ctx, pi, po, float(dt), int(nstages), pw))
+
+    def sync(self):
+        self._check(lib().chorus_sync(self._ctx))
 
     def diagnostics_sums(self):
         out = np.empty(3)

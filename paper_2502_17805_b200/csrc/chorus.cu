@@ -69,6 +69,17 @@ struct chorus_ctx {
   bool prof = false;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[3];
   std::string err;
+  struct HostPipe* pipe = nullptr;   // chorus_step_host: copy streams, staging buffers and events (made on first use)
+};
+
+// Pipelined host jobs (chorus_step_host): job k uses slot k % 2 of every array.
+struct HostPipe {
+  cudaStream_t s_in = nullptr, s_out = nullptr;          // host -> device and device -> host copies
+  double* in[2] = {nullptr, nullptr};                    // staged inputs  [9][E][n3] (interface layout)
+  double* out[2] = {nullptr, nullptr};                   // staged results [9][E][n3]
+  unsigned long long* ws[2] = {nullptr, nullptr};        // wave speed of the result (bits of a double)
+  cudaEvent_t in_ready[2] = {}, in_free[2] = {}, out_ready[2] = {}, out_free[2] = {};
+  int64_t jobs = 0;
 };
 
 namespace {
@@ -489,6 +500,20 @@ void chorus_free(chorus_ctx* c) {
       cudaEventDestroy(ev.first);
       cudaEventDestroy(ev.second);
     }
+  if (HostPipe* hp = c->pipe) {
+    if (hp->s_in) cudaStreamSynchronize(hp->s_in);
+    if (hp->s_out) cudaStreamSynchronize(hp->s_out);
+    for (int k = 0; k < 2; ++k) {
+      cudaFree(hp->in[k]); cudaFree(hp->out[k]); cudaFree(hp->ws[k]);
+      if (hp->in_ready[k]) cudaEventDestroy(hp->in_ready[k]);
+      if (hp->in_free[k]) cudaEventDestroy(hp->in_free[k]);
+      if (hp->out_ready[k]) cudaEventDestroy(hp->out_ready[k]);
+      if (hp->out_free[k]) cudaEventDestroy(hp->out_free[k]);
+    }
+    if (hp->s_in) cudaStreamDestroy(hp->s_in);
+    if (hp->s_out) cudaStreamDestroy(hp->s_out);
+    delete hp;
+  }
   delete c;
 }
 
@@ -635,6 +660,84 @@ int chorus_step(chorus_ctx* c, double dt, int nstages) {
   }
   c->cur = a.cur_after;
   guard.ok = true;
+  return CHORUS_OK;
+}
+
+// ---- host jobs, pipelined: H2D of job k + 1 and D2H of job k - 1 run beside the kernels of job k
+namespace {
+int host_pipe(chorus_ctx* c, HostPipe** out) {
+  if (!c->pipe) {
+    HostPipe* hp = new HostPipe;
+    c->pipe = hp;                    // chorus_free releases whatever was made, also after a failure below
+    const size_t count = (size_t)c->E * 9 * c->n3;
+    CU(c, cudaStreamCreateWithFlags(&hp->s_in, cudaStreamNonBlocking));
+    CU(c, cudaStreamCreateWithFlags(&hp->s_out, cudaStreamNonBlocking));
+    for (int k = 0; k < 2; ++k) {
+      if (cudaMalloc(&hp->in[k], sizeof(double) * count) != cudaSuccess || cudaMalloc(&hp->out[k], sizeof(double) * count) != cudaSuccess ||
+          cudaMalloc(&hp->ws[k], sizeof(unsigned long long)) != cudaSuccess)
+        return fail(c, CHORUS_ENOMEM, "chorus_step_host: staging buffers");
+      CU(c, cudaEventCreateWithFlags(&hp->in_ready[k], cudaEventDisableTiming));
+      CU(c, cudaEventCreateWithFlags(&hp->in_free[k], cudaEventDisableTiming));
+      CU(c, cudaEventCreateWithFlags(&hp->out_ready[k], cudaEventDisableTiming));
+      CU(c, cudaEventCreateWithFlags(&hp->out_free[k], cudaEventDisableTiming));
+    }
+  }
+  if (!c->pipe->out_free[1]) return fail(c, CHORUS_ESTATE, "chorus_step_host: the pipeline could not be set up earlier");
+  *out = c->pipe;
+  return CHORUS_OK;
+}
+}  // namespace
+
+int chorus_step_host(chorus_ctx* c, const double* q_in, double* q_out, double dt, int nstages, double* ws_out) {
+  if (!c || !q_in || !q_out) return CHORUS_EINVAL;
+  if ((nstages != 1 && nstages != 3 && nstages != 5) || !(dt == dt)) return fail(c, CHORUS_EINVAL, "bad dt or nstages");
+  if (c->E_own != c->E) return fail(c, CHORUS_EINVAL, "chorus_step_host serves unpartitioned contexts");
+  if (c->split_next >= 0) return fail(c, CHORUS_ESTATE, "a split step is in progress");
+  HostPipe* hp = nullptr;
+  if (int rc = host_pipe(c, &hp)) return rc;
+  const int k = (int)(hp->jobs & 1);
+  const bool reuse = hp->jobs >= 2;                       // slot k was last used by job jobs - 2
+  const size_t count = (size_t)c->E * 9 * c->n3;
+  // copy-in stream: the staged input of slot k must have been consumed (transposed into the state registers) by its last job
+  if (reuse) CU(c, cudaStreamWaitEvent(hp->s_in, hp->in_free[k], 0));
+  CU(c, cudaMemcpyAsync(hp->in[k], q_in, sizeof(double) * count, cudaMemcpyHostToDevice, hp->s_in));
+  CU(c, cudaEventRecord(hp->in_ready[k], hp->s_in));
+  // the context's stream: state in, one step, state (and wave speed) out
+  CU(c, cudaStreamWaitEvent(c->stream, hp->in_ready[k], 0));
+  to_element_major<<<grid_1d(c, (int64_t)count, 256), 256, 0, c->stream>>>(c->E, c->n3, 9, hp->in[k], c->d_U[0]);
+  ++c->launches;
+  CU(c, cudaGetLastError());
+  CU(c, cudaEventRecord(hp->in_free[k], c->stream));
+  c->cur = 0;
+  c->have_state = true;
+  c->traces_valid = false;
+  if (int rc = chorus_step(c, dt, nstages)) return rc;
+  if (reuse) CU(c, cudaStreamWaitEvent(c->stream, hp->out_free[k], 0));      // the D2H of slot k's last result has finished
+  from_element_major<<<grid_1d(c, (int64_t)count, 256), 256, 0, c->stream>>>(c->E, c->n3, 9, c->d_U[c->cur], hp->out[k]);
+  ++c->launches;
+  CU(c, cudaGetLastError());
+  if (ws_out) {
+    CU(c, cudaMemsetAsync(hp->ws[k], 0, sizeof(unsigned long long), c->stream));
+    const int64_t total = c->E * c->n3;
+    wavespeed_kernel<<<grid_1d(c, total, 256), 256, 0, c->stream>>>(c->E, c->n3, c->ph, c->d_U[c->cur], hp->ws[k]);
+    ++c->launches;
+    CU(c, cudaGetLastError());
+  }
+  CU(c, cudaEventRecord(hp->out_ready[k], c->stream));
+  // copy-out stream
+  CU(c, cudaStreamWaitEvent(hp->s_out, hp->out_ready[k], 0));
+  CU(c, cudaMemcpyAsync(q_out, hp->out[k], sizeof(double) * count, cudaMemcpyDeviceToHost, hp->s_out));
+  if (ws_out) CU(c, cudaMemcpyAsync(ws_out, hp->ws[k], sizeof(double), cudaMemcpyDeviceToHost, hp->s_out));
+  CU(c, cudaEventRecord(hp->out_free[k], hp->s_out));
+  ++hp->jobs;
+  return CHORUS_OK;
+}
+
+int chorus_sync(chorus_ctx* c) {
+  if (!c) return CHORUS_EINVAL;
+  if (c->pipe && c->pipe->s_in) CU(c, cudaStreamSynchronize(c->pipe->s_in));
+  CU(c, cudaStreamSynchronize(c->stream));
+  if (c->pipe && c->pipe->s_out) CU(c, cudaStreamSynchronize(c->pipe->s_out));
   return CHORUS_OK;
 }
 

@@ -28,7 +28,7 @@ def _case(n, nz, nr, diff, seed=31):
     return w, mesh, g, Q, phys, w.dt(g.max_wavespeed(), xf[1] - xf[0])
 
 
-@pytest.mark.parametrize("n,diff", [(6, 1e-3), (6, 0.0), (4, 1e-3), (5, 0.0), (7, 1e-3)])
+@pytest.mark.parametrize("n,diff", [(6, 1e-3), (6, 0.0), (4, 1e-3), (5, 0.0), (7, 1e-3), (8, 1e-3)])
 def test_results_do_not_depend_on_the_number_of_partitions(n, diff):
     w, mesh, g, Q, phys, dt = _case(n, 6, 3, diff)
     for _ in range(2):

@@ -78,8 +78,23 @@ struct Mma {
     const int a = ab % N, b = ab / N;
     return d == 0 ? (b == 0 && a < LO) : d == 1 ? (b == 1 && a < LO) : (a >= LO && b >= LO && (b - LO) * (N - LO) + (a - LO) < LO);
   }
-  // slot 0 .. 8 FG - 1: the lines that are not left over, in increasing order; slot 8 FG + i: the i-th left-over line
+  // slot 0 .. 8 FG - 1: the lines that are not left over, in increasing order; slot 8 FG + i: the i-th left-over line.
+  // n = 6: the full groups are ordered so that the four lines of a half-warp (rows r = 0..3, r = 4..7) start in shared-memory
+  // banks that the 4 k-offsets of an A-operand load tile without overlap (a 64-bit load serves 16 lanes per wavefront over 16
+  // double-wide banks): direction 0 (line pitch 6, k-offsets 0..3): bases 6 ab = {0,4,8,12} or {2,6,10,14} mod 16, i.e. four
+  // even or four odd ab; direction 1 (bases 36 b + a, k-offsets {0,6,12,18}): bases {k, k+1, k+8, k+9} mod 16, i.e. lines (a,b),
+  // (a+1,b), (a,b+2), (a+1,b+2); direction 2 (bases ab, k-offsets {0,4,8,12}) is conflict-free as it stands.
   __host__ __device__ static constexpr int line_of(int d, int slot) {
+    if (N == 6 && slot < 8 * FG) {
+      if (d == 0) {
+        const int g = slot / 8, r = slot % 8;
+        return 4 + 8 * g + (r < 4 ? 2 * r : 2 * (r - 4) + 1);
+      }
+      if (d == 1) {
+        constexpr int t[32] = {0, 1, 12, 13, 2, 3, 14, 15, 4, 5, 16, 17, 10, 11, 22, 23, 18, 19, 30, 31, 20, 21, 32, 33, 24, 25, 34, 35, 26, 27, 28, 29};
+        return t[slot];
+      }
+    }
     int cnt = 0, lo = 0;
     for (int ab = 0; ab < I::n2; ++ab) {
       if (is_lo(d, ab)) {

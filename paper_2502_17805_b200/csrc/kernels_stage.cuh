@@ -651,6 +651,10 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
   constexpr int kGS = ev(3 * NGV * I::n3);
   double* sR12 = sG + (kPre ? 2 : 1) * kGS;  // kFree: the accumulators of directions 1 and 2, [2][9][n3] (direction 0: sR);
   constexpr int kRS = ev(9 * I::n3);         // kPre: the two accumulators of the two task waves (see the chain loop)
+  // kPre without diffusion, step mode: the new state of the finished element, from which its face traces are made -- by the
+  // chain warps, in the time they would otherwise wait for the next gradient (without diffusion the helpers are the longer side)
+  double* sNew = sR12 + 2 * kRS;
+  constexpr bool kChainTraces = kPre && !DIFF;
   __shared__ ElemNbr nbs[2];
   __shared__ int s_second;
   __shared__ int s_task[kPre ? M::kTasks * 8 : 1];   // kPre: (task, row) -> line | direction << 16 | row carries a line << 20
@@ -847,8 +851,10 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           // The bulk copies of the next element are observed BEFORE this warp reports that it is done with element e: after
           // that report the helpers may start the copies of the element after the next, and a wait for "the phase of this
           // parity" would then match the wrong phase.
+          if (kChainTraces && io.Qout != nullptr && it > 0)     // traces of the element before, whose new state the helpers left in sNew
+            emit_traces<N>(sNew, io.QfOut + (e - gridDim.x) * 54 * I::n2, tid, 32 * kGW0);
           if (more) wait_inputs();
-          bar_arrive(kBarRes, kMainThreads);     // this warp is done with element e
+          bar_arrive(kBarRes, kMainThreads);     // this warp is done with element e (and with sNew)
           if (!more) break;
           load_jv(e + gridDim.x);
         } else {
@@ -879,6 +885,11 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         chain_rule(sG + (cur ^ 1) * kGS);
         bar_sync(kBarChain, CH);
         bar_arrive(kBarGrad, kMainThreads);
+      }
+      if (kChainTraces && io.Qout != nullptr && (int64_t)blockIdx.x < E) {   // the last element's traces, once the helpers have finished it
+        const int64_t e_last = (int64_t)blockIdx.x + (int64_t)it * gridDim.x;
+        bar_sync(kBarIn, kMainThreads);
+        emit_traces<N>(sNew, io.QfOut + e_last * 54 * I::n2, tid, CH);
       }
     } else
     for (int64_t e = blockIdx.x; e < E; e += gridDim.x, ++it) {
@@ -1111,7 +1122,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
 #pragma unroll
             for (int v = 0; v < 9; ++v) {
               io.Qout[(ef * 9 + v) * I::n3 + s] = R[v];
-              sQ[v * I::n3 + s] = R[v];   // this thread is the only reader and writer of point s in this phase
+              (kChainTraces ? sNew : sQ)[v * I::n3 + s] = R[v];   // this thread is the only reader and writer of point s in this phase
             }
           } else {
 #pragma unroll
@@ -1119,7 +1130,7 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
           }
         }
       }
-      if (!DIFF && rk) {
+      if (!DIFF && rk && !kChainTraces) {
         bar_sync(kBarHelp, H);
         emit_traces<N>(sQ, io.QfOut + ef * 54 * I::n2, tid, H);
       }
@@ -1210,10 +1221,12 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         const int cur = it & 1;
         const bool more = e + gridDim.x < E;
         e_last = e;
-        // The chain warps are done with the previous element (RES): its input set is free.  With diffusion its finish touches no
-        // input tile (it writes Part from the accumulators): the next loads go first, so that the proxy fence of their issuing
-        // threads does not wait for the finish's global stores.  The single neighbour tile is free as well: the chain warps
-        // report RES after the gradient tasks that read it -- except before the first element, whose gradient is awaited here.
+        // The chain warps are done with the previous element (RES): its input set is free, and its finish touches no input tile
+        // (it reads the accumulators and writes global memory, without diffusion also sNew).  With diffusion the next loads go
+        // first, so that the proxy fence of their issuing threads does not wait for the finish's global stores (the chain warps
+        // need the accumulators only after the streamed viscous flux of their first task); without it the chain warps need them
+        // almost at once, and the finish goes first.  The single neighbour tile is free as well: the chain warps report RES after
+        // the gradient tasks that read it -- except before the first element, whose gradient is awaited here.
         if (it == 0) bar_sync(kBarGrad, kMainThreads);
         if (DIFF && more) {
           issue_loads_a(e + gridDim.x, cur ^ 1);
@@ -1240,7 +1253,10 @@ stage_main_kernel(int64_t E, PhysD ph, StageIO io, Geo geo) {
         sources(e, sm + cur * kIn, sG + cur * kGS);
         bar_sync(kBarRes, kMainThreads);             // every chain warp is done with element e
       }
-      if (e_last >= 0) finish(e_last, (it - 1) & 1);
+      if (e_last >= 0) {
+        finish(e_last, (it - 1) & 1);
+        if (kChainTraces && rk) bar_arrive(kBarIn, kMainThreads);      // the chain warps make the last element's traces
+      }
     } else
 
     for (int64_t e = blockIdx.x; e < E; e += gridDim.x, ++it) {
@@ -1404,7 +1420,8 @@ constexpr size_t stage_main_smem_bytes() {
   constexpr auto ev = [](int x) { return (x + 1) & ~1; };
   constexpr int kST = kSglobalOrder(N) ? 0 : kSintOrder(N) ? 9 * I::n2 * (N - 1) : 9 * I::nf;
   if (kPrefetchOrder(N))   // two sets of (state, own traces / fluxes, S^d), one neighbour tile, two gradients, two accumulators
-    return sizeof(double) * (size_t)(2 * (ev(9 * I::n3) + ev(kOwn) + kST) + ev(54 * I::n2) + 2 * ev(3 * NGV * I::n3) + 2 * ev(9 * I::n3));
+    return sizeof(double) * (size_t)(2 * (ev(9 * I::n3) + ev(kOwn) + kST) + ev(54 * I::n2) + 2 * ev(3 * NGV * I::n3) + 2 * ev(9 * I::n3) +
+                                     (GRADV != 2 ? ev(9 * I::n3) : 0));      // without diffusion: the new-state tile sNew
   return sizeof(double) * (size_t)((kPrefetchOrder(N) ? 2 : 1) * (ev(9 * I::n3) + ev(kOwn) + ev(54 * I::n2) + kST) +
                                    (kPrefetchOrder(N) ? 2 : 1) * ev(3 * NGV * I::n3) + (Mma<N>::kFree ? 2 * ev(9 * I::n3) : 0));
 }

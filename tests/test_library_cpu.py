@@ -72,3 +72,26 @@ def test_product_package_does_not_touch_the_oracle():
         if f.endswith((".cpp", ".h")):
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "csrc" not in src.replace("paper_2502_17805_b200/csrc).", "") and "#include \"../" not in src
+
+
+def test_context_free_entry_points_reject_bad_arguments_without_a_device():
+    """chorus_diagnostics_static validates its arguments before it touches the device: bad order, empty mesh, null pointers and a
+    size beyond the static scratch's maximum come back as CHORUS_EINVAL with a message; chorus_step_host / chorus_sync refuse a
+    null context.  (No compute call is made: there is no GPU here.)"""
+    L = P.lib()
+    buf = (C.c_double * 4)()
+    p = C.cast(buf, C.c_void_p)
+    assert L.chorus_diagnostics_static(10, 1, p, p, p, None) == B.CHORUS_EINVAL
+    assert b"order" in L.chorus_static_last_error()
+    assert L.chorus_diagnostics_static(6, 0, p, p, p, None) == B.CHORUS_EINVAL
+    assert L.chorus_diagnostics_static(6, 1, None, p, p, None) == B.CHORUS_EINVAL
+    too_many = B.STATIC_DIAG_MAX_POINTS // 216 + 1
+    assert L.chorus_diagnostics_static(6, too_many, p, p, p, None) == B.CHORUS_EINVAL
+    msg = L.chorus_static_last_error().decode()
+    assert "maximum" in msg and str(B.STATIC_DIAG_MAX_POINTS) in msg
+    assert L.chorus_step_host(None, p, p, 1e-3, 5, None) == B.CHORUS_EINVAL
+    assert L.chorus_sync(None) == B.CHORUS_EINVAL
+    import torch
+    with pytest.raises(P.ChorusError):
+        P.diagnostics_static(6, torch.zeros(9, 1, 216, dtype=torch.float64), torch.zeros(1, 216, dtype=torch.float64),
+                             torch.zeros(3, dtype=torch.float64))
